@@ -1,0 +1,170 @@
+/*
+ * hfft.h -- C ABI of the B200-native hybrid-FFT demagnetization field library.
+ *
+ * Method: Heistracher et al., "Hybrid FFT algorithm for fast demagnetization
+ * field calculations on non-equidistant magnetic layers", arXiv 1910.07054.
+ * Citations are PAPER.md:<line> (+ equation); readings A1..A16 are listed in
+ * DESIGN.md.
+ *
+ * What the library computes (Eq.18 with PAPER.md:150 Eq.19):
+ *
+ *   H_a(a1,a2,i) = - sum_j Ms_j sum_{b1,b2} sum_b N^{ab}_{ij}((a1-b1)dx,(a2-b2)dy) m_b(b1,b2,j)
+ *
+ * for nz layers of nx x ny cells with common in-plane cell size dx x dy and a
+ * per-layer thickness dz[j], N_ij the generalized Newell
+ * tensor of two cuboids of unequal thickness (PAPER.md:52 Eq.5, :99 Eq.11,
+ * :249-291 Eq.27-31).  It is evaluated with the paper's hybrid scheme
+ * (Eq.24): 2-D FFT in the plane (zero-padded to 2nx x 2ny),
+ * explicit layer-to-layer convolution along z at every in-plane wavevector,
+ * inverse 2-D FFT, crop.
+ *
+ * Everything runs on ONE CUDA device (sm_100a), in hand-written kernels; there
+ * is no cuFFT, no CPU fallback and no collective.  Every call returns a status;
+ * nothing throws across this boundary.  A plan is not thread-safe.
+ *
+ * Array layout (all calls): [B][3][nz][ny][nx], x fastest, component order
+ * (x,y,z), element type float (HFFT_F32) or double (HFFT_F64), 16-byte aligned.
+ */
+#ifndef HFFT_H
+#define HFFT_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hfft_plan hfft_plan; /* opaque */
+
+typedef enum { HFFT_F32 = 0, HFFT_F64 = 1 } hfft_precision;
+
+typedef enum {
+    HFFT_OK = 0,
+    HFFT_EINVAL = 1,       /* bad argument (null, non-positive or non-finite size, misaligned pointer) */
+    HFFT_ENOMEM = 2,       /* device or host allocation failed */
+    HFFT_ECUDA = 3,        /* a CUDA runtime call or kernel launch failed; see hfft_last_error */
+    HFFT_ESTATE = 4,       /* call out of order (e.g. hfft_demag before hfft_build_tensor) */
+    HFFT_EUNSUPPORTED = 5  /* nx or ny not a power of two, nz above HFFT_MAX_NZ, no sm_100 device */
+} hfft_status;
+
+#define HFFT_MAX_NZ 256
+
+/* Stage indices of the hot path. */
+enum { HFFT_STAGE_FFTX = 0, HFFT_STAGE_FFTY = 1, HFFT_STAGE_COUPLING = 2,
+       HFFT_STAGE_IFFTY = 3, HFFT_STAGE_IFFTX = 4, HFFT_NUM_STAGES = 5 };
+
+/* Geometry and derived sizes of a plan (filled by hfft_plan_info). */
+typedef struct {
+    int nx, ny, nz, batch;
+    int precision;            /* hfft_precision */
+    int tile_k;               /* wavevectors per bank tile */
+    long long n_k;            /* wavevectors in the Hermitian half spectrum: (nx+1) * 2ny */
+    long long n_k_padded;     /* n_k rounded up to a multiple of tile_k */
+    size_t bank_bytes;        /* spectral tensor bank: 6 * nz^2 * n_k_padded * sizeof(element) */
+    size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging */
+    size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
+    int launches_per_demag;   /* kernels hfft_demag enqueues per call */
+    int built;                /* 1 once hfft_build_tensor has completed */
+} hfft_info;
+
+/*
+ * Create a plan for nz layers of nx x ny cells (common dx, dy;
+ * layer k has thickness dz[k]; layers are stacked contiguously in array order,
+ * reading A9).  dz is a HOST array of nz doubles and is copied.  Lengths are in
+ * any one unit (the tensor depends on ratios only).  Selects device = the
+ * current CUDA device.  No device memory is allocated here.
+ * Errors: EINVAL (null out/dz, nx,ny < 2, nz < 1, non-positive or non-finite
+ * dx, dy, dz[k]); EUNSUPPORTED (nx or ny not a power of two, nz > HFFT_MAX_NZ,
+ * device is not compute capability 10.x); ENOMEM.
+ */
+hfft_status hfft_plan_create(hfft_plan **out, int nx, int ny, int nz,
+                             double dx, double dy, const double *dz, hfft_precision precision);
+
+/* Number of independent magnetisation states per hfft_demag call (default 1;
+ * BASELINE config 5 uses 32).  Must be called before hfft_build_tensor /
+ * hfft_plan_set_buffers.  Errors: EINVAL (B < 1), ESTATE. */
+hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
+
+/* Sizes the plan needs; valid after create / set_batch.  Errors: EINVAL. */
+hfft_status hfft_plan_info(const hfft_plan *plan, hfft_info *info);
+
+/*
+ * Optional: hand the plan caller-owned DEVICE buffers (e.g. torch tensors) of
+ * at least info.bank_bytes and info.workspace_bytes, 256-byte aligned.  The
+ * caller keeps ownership and must keep them alive until hfft_destroy.  Without
+ * this call hfft_build_tensor allocates both with cudaMalloc and hfft_destroy
+ * frees them.  Errors: EINVAL, ESTATE (after build).
+ */
+hfft_status hfft_plan_set_buffers(hfft_plan *plan, void *bank, void *workspace);
+
+/*
+ * Timed setup.  On device: evaluates the generalized Newell
+ * tensor N^{ab}_{ij}(p dx, q dy) for every layer pair and in-plane offset
+ * (PAPER.md:52 Eq.5, :99 Eq.11 with the 4th term read as Y+dy [A1], :80-85
+ * Eq.10, :123-132 Eq.16, other components by permutation PAPER.md:46) in
+ * double-double arithmetic (the 64-term sums cancel catastrophically in plain
+ * fp64, reading A16), places it on the 2nx x 2ny periodic grid (A10), takes its
+ * in-plane FFT in fp64 (left factor of PAPER.md:177 Eq.24) and stores the real
+ * (xx,yy,zz,xy) or imaginary (xz,yz) part in the plan precision.
+ * Enqueues on `stream` (a cudaStream_t, may be NULL = default stream) and
+ * synchronises that stream before returning (it frees its scratch memory).
+ * Errors: ENOMEM, ECUDA.
+ */
+hfft_status hfft_build_tensor(hfft_plan *plan, void *stream);
+
+/*
+ * The hot path: one demagnetization-field evaluation (Eq.24).
+ *   m   DEVICE pointer, [B][3][nz][ny][nx], plan precision, read only
+ *   Ms  HOST pointer to nz doubles (per-layer saturation magnetisation, Eq.17
+ *       PAPER.md:140, per-layer by reading A12), read during the call and passed
+ *       by value to the kernels; NULL means 1.0 (m already holds M)
+ *   h   DEVICE pointer, same shape and type as m, overwritten; units of Ms;
+ *       must not alias m
+ * Only enqueues kernels on `stream`: no host synchronisation, no allocation,
+ * safe to capture in a CUDA graph.  Errors: EINVAL, ESTATE (tensor not built),
+ * ECUDA (launch failure).
+ */
+hfft_status hfft_demag(hfft_plan *plan, const void *m, const double *Ms, void *h, void *stream);
+
+/*
+ * Same evaluation with HOST buffers (pinned memory gives asynchronous copies):
+ * copies m to a staging buffer inside the plan workspace, runs hfft_demag,
+ * copies h back, all on `stream`.  Does not synchronise the stream.
+ */
+hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *Ms, void *h_host,
+                            void *stream);
+
+/*
+ * Per-stage device timing.  With profiling on, hfft_demag brackets every stage
+ * with CUDA events on `stream`.  hfft_profile_read synchronises on the last
+ * event and returns, for each of the HFFT_NUM_STAGES stages, the SUM of elapsed
+ * milliseconds over the calls since the last read, and the number of calls; it
+ * then resets the sums.  At most 256 calls are kept between reads (further
+ * calls return ESTATE).  Profiling makes hfft_demag unsuitable for graph capture.
+ */
+hfft_status hfft_profile_enable(hfft_plan *plan, int on);
+hfft_status hfft_profile_read(hfft_plan *plan, double stage_ms[HFFT_NUM_STAGES], int *calls);
+
+/*
+ * Introspection for tests: copy one spectral bank plane N^_{ij}^{c}(k) to a
+ * HOST array of n_k doubles, c in xx,yy,zz,xy,xz,yz = 0..5.  Element k =
+ * ky * nx + kx for kx < nx, and 2ny * nx + ky for the Nyquist column kx = nx.
+ * The value is the real part for c < 4 and the imaginary part for c = 4, 5.
+ * Synchronises the device.  Errors: EINVAL, ESTATE.
+ */
+hfft_status hfft_read_bank(const hfft_plan *plan, int i, int j, int c, double *out_host);
+
+/* Release the plan and everything it owns.  NULL is allowed. */
+hfft_status hfft_destroy(hfft_plan *plan);
+
+/* Message of the last failing call on this plan ("" if none); plan may be NULL
+ * to get the message of the last failing hfft_plan_create on this thread. */
+const char *hfft_last_error(const hfft_plan *plan);
+
+/* Library build identification, e.g. "hfft 0.1 sm_100a". */
+const char *hfft_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HFFT_H */

@@ -1,0 +1,192 @@
+// coupling.cu -- stage S3: the explicit layer-to-layer convolution along z at every in-plane
+// wavevector, the sum over j3 of Eq.24:
+//
+//     H^_i(k) = - sum_j N^_ij(k) M^_j(k),    N^_ij(k) a symmetric 3x3 tensor per layer pair,
+//
+// "the remaining convolution in the third dimension has to be calculated explicitly";
+// it is the O(nz^2) term of the method.
+//
+// Real form: xx,yy,zz,xy spectra are purely real (A), xz,yz purely imaginary
+// (i B).  With M'_z = i M_z and H'_z = i H_z the coupling is the REAL matrix
+//     [Hx ; Hy ; H'z] = [[a0, a3, a4], [a3, a1, a5], [-a4, -a5, a2]] [Mx ; My ; M'z]
+// acting on real and imaginary parts alike, where the bank stores, per (i, j, k),
+//     a0..a5 = -s (Axx, Ayy, Azz, Axy, Bxz, Byz),  s = 1/(4 nx ny)  (sign and normalisation folded).
+//
+// Bank layout: [tile][i][j][6][tile_k] elements of T; one CTA item = one k-tile of one state.
+// A warp owns one target layer i at a time; a lane owns KPT consecutive wavevectors, so each
+// bank access of a warp is one fully coalesced 32*KPT*sizeof(T)-byte request (512 B at KPT = 4),
+// and the whole [i][j][6] stream of a tile is contiguous in memory.  M^ of all layers for the
+// tile sits in shared memory (cp.async, 16-byte chunks, XOR-swizzled against bank conflicts);
+// H^ overwrites M^ in place (each tile is read completely before it is written).
+#include "hfft_internal.h"
+#include "fft.cuh"
+
+namespace hfft {
+
+template <typename T, int KPT> struct BankVec;
+template <> struct BankVec<float, 4> {
+    static __device__ __forceinline__ void ld(const float* p, float v[4]) {
+        float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+        v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
+    }
+};
+template <> struct BankVec<float, 1> {
+    static __device__ __forceinline__ void ld(const float* p, float v[1]) { v[0] = __ldcs(p); }
+};
+template <> struct BankVec<double, 2> {
+    static __device__ __forceinline__ void ld(const double* p, double v[2]) {
+        double2 t = __ldcs(reinterpret_cast<const double2*>(p));
+        v[0] = t.x; v[1] = t.y;
+    }
+};
+template <> struct BankVec<double, 1> {
+    static __device__ __forceinline__ void ld(const double* p, double v[1]) { v[0] = __ldcs(p); }
+};
+
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
+    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc));
+}
+__device__ __forceinline__ void cp_async_wait_all() {
+    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
+}
+
+template <typename T, int KPT>
+__global__ void __launch_bounds__(512)
+coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
+                long long ks) {
+    typedef HFFT_C C;
+    constexpr int TK = 32 * KPT;
+    constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk (2 or 1)
+    constexpr int CPP = TK / CHUNK_C;                     // chunks per plane row
+    constexpr bool SWZ = (KPT * sizeof(C) == 32);         // two 16-byte chunks per lane
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* sm = reinterpret_cast<C*>(smem_raw);               // [3 nz][TK] (chunk-swizzled)
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
+    const int np = 3 * nz;
+    const long long n_items = n_tiles * batch;
+
+    for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const long long tile = item / batch;
+        const int b = (int)(item - tile * batch);
+        C* sp = spec + (long long)b * np * ks + tile * TK;
+
+        for (int w = tid; w < np * CPP; w += blockDim.x) {
+            const int lp = w / CPP, ch = w - lp * CPP;
+            const int chs = SWZ ? (ch ^ ((ch >> 3) & 1)) : ch;
+            cp_async16(sm + lp * TK + chs * CHUNK_C, sp + (long long)lp * ks + ch * CHUNK_C);
+        }
+        cp_async_wait_all();
+        __syncthreads();
+
+        for (int i = warp; i < nz; i += nwarps) {
+            T hx[KPT][2], hy[KPT][2], hz[KPT][2];
+#pragma unroll
+            for (int e = 0; e < KPT; ++e) { hx[e][0] = hx[e][1] = hy[e][0] = hy[e][1] = hz[e][0] = hz[e][1] = (T)0; }
+            const T* bt = bank + ((tile * nz + i) * nz) * (6LL * TK) + lane * KPT;
+#pragma unroll 2
+            for (int j = 0; j < nz; ++j) {
+                T a[6][KPT];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) BankVec<T, KPT>::ld(bt + (j * 6 + c) * TK, a[c]);
+                C m[3][KPT];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    const C* row = sm + (c * nz + j) * TK;
+                    if (SWZ) {
+                        // lane owns chunks 2*lane and 2*lane+1 of the row
+                        const int c0 = 2 * lane, c1 = 2 * lane + 1;
+                        const int s0 = c0 ^ ((c0 >> 3) & 1), s1 = c1 ^ ((c1 >> 3) & 1);
+                        if (sizeof(T) == 4) {
+                            float4 u0 = *reinterpret_cast<const float4*>(row + s0 * CHUNK_C);
+                            float4 u1 = *reinterpret_cast<const float4*>(row + s1 * CHUNK_C);
+                            m[c][0] = mk<T>(u0.x, u0.y); m[c][1 % KPT] = mk<T>(u0.z, u0.w);
+                            m[c][2 % KPT] = mk<T>(u1.x, u1.y); m[c][3 % KPT] = mk<T>(u1.z, u1.w);
+                        } else {
+                            m[c][0] = row[s0 * CHUNK_C];
+                            m[c][1 % KPT] = row[s1 * CHUNK_C];
+                        }
+                    } else {
+#pragma unroll
+                        for (int e = 0; e < KPT; ++e) m[c][e] = row[lane * KPT + e];
+                    }
+                }
+#pragma unroll
+                for (int e = 0; e < KPT; ++e) {
+                    hx[e][0] += a[0][e] * m[0][e].x + a[3][e] * m[1][e].x + a[4][e] * m[2][e].x;
+                    hx[e][1] += a[0][e] * m[0][e].y + a[3][e] * m[1][e].y + a[4][e] * m[2][e].y;
+                    hy[e][0] += a[3][e] * m[0][e].x + a[1][e] * m[1][e].x + a[5][e] * m[2][e].x;
+                    hy[e][1] += a[3][e] * m[0][e].y + a[1][e] * m[1][e].y + a[5][e] * m[2][e].y;
+                    hz[e][0] += a[2][e] * m[2][e].x - a[4][e] * m[0][e].x - a[5][e] * m[1][e].x;
+                    hz[e][1] += a[2][e] * m[2][e].y - a[4][e] * m[0][e].y - a[5][e] * m[1][e].y;
+                }
+            }
+            C* ox = sp + (long long)(0 * nz + i) * ks + lane * KPT;
+            C* oy = sp + (long long)(1 * nz + i) * ks + lane * KPT;
+            C* oz = sp + (long long)(2 * nz + i) * ks + lane * KPT;
+            if (SWZ && sizeof(T) == 4) {
+                reinterpret_cast<float4*>(ox)[0] = make_float4(hx[0][0], hx[0][1], hx[1 % KPT][0], hx[1 % KPT][1]);
+                reinterpret_cast<float4*>(ox)[1] = make_float4(hx[2 % KPT][0], hx[2 % KPT][1], hx[3 % KPT][0], hx[3 % KPT][1]);
+                reinterpret_cast<float4*>(oy)[0] = make_float4(hy[0][0], hy[0][1], hy[1 % KPT][0], hy[1 % KPT][1]);
+                reinterpret_cast<float4*>(oy)[1] = make_float4(hy[2 % KPT][0], hy[2 % KPT][1], hy[3 % KPT][0], hy[3 % KPT][1]);
+                reinterpret_cast<float4*>(oz)[0] = make_float4(hz[0][0], hz[0][1], hz[1 % KPT][0], hz[1 % KPT][1]);
+                reinterpret_cast<float4*>(oz)[1] = make_float4(hz[2 % KPT][0], hz[2 % KPT][1], hz[3 % KPT][0], hz[3 % KPT][1]);
+            } else {
+#pragma unroll
+                for (int e = 0; e < KPT; ++e) {
+                    ox[e] = mk<T>(hx[e][0], hx[e][1]);
+                    oy[e] = mk<T>(hy[e][0], hy[e][1]);
+                    oz[e] = mk<T>(hz[e][0], hz[e][1]);
+                }
+            }
+        }
+        __syncthreads();   // every warp is done with the tile in shared memory
+    }
+}
+
+size_t coupling_smem_bytes(int nz, int tile_k, size_t elem) { return (size_t)3 * nz * tile_k * 2 * elem; }
+
+template <typename T, int KPT>
+static cudaError_t launch_coupling_k(const void* bank, void* spec, int nz, int batch, long long n_tiles, long long ks,
+                                     int num_sms, cudaStream_t st) {
+    typedef HFFT_C C;
+    auto kern = coupling_kernel<T, KPT>;
+    const size_t smem = coupling_smem_bytes(nz, 32 * KPT, sizeof(T));
+    const int warps = nz < 16 ? nz : 16;
+    const int threads = warps * 32;
+    static size_t smem_done = 0;
+    static int occ_threads = 0, occ_blocks = 0;
+    static size_t occ_smem = 0;
+    cudaError_t err;
+    if (smem > 48 * 1024 && smem > smem_done) {
+        err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        smem_done = smem;
+    }
+    if (occ_threads != threads || occ_smem != smem) {
+        int nb = 0;
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
+        if (err != cudaSuccess) return err;
+        occ_threads = threads; occ_smem = smem; occ_blocks = nb < 1 ? 1 : nb;
+    }
+    long long items = n_tiles * batch;
+    long long grid = (long long)num_sms * occ_blocks;
+    if (grid > items) grid = items;
+    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)bank, (C*)spec, nz, batch, n_tiles, ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
+                            long long ks, int num_sms, cudaStream_t st) {
+    constexpr int KV = 16 / sizeof(T);
+    if (tile_k == 32 * KV) return launch_coupling_k<T, KV>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
+    if (tile_k == 32) return launch_coupling_k<T, 1>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
+    return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_coupling<float>(const void*, void*, int, int, int, long long, long long, int, cudaStream_t);
+template cudaError_t launch_coupling<double>(const void*, void*, int, int, int, long long, long long, int, cudaStream_t);
+
+}  // namespace hfft

@@ -1,0 +1,371 @@
+// hfft_api.cu -- the C ABI declared in include/hfft.h: plan object, argument checks, twiddle
+// tables, stage orchestration.  No arithmetic of the method lives here except the twiddle table.
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "hfft_internal.h"
+
+using namespace hfft;
+
+namespace {
+thread_local std::string g_create_error;
+constexpr int kMaxProfileCalls = 256;
+}  // namespace
+
+struct hfft_plan {
+    int nx = 0, ny = 0, nz = 0, batch = 1, log2nx = 0, log2ny = 0;
+    hfft_precision prec = HFFT_F32;
+    double dx = 0, dy = 0;
+    std::vector<double> dz;
+    int device = 0, num_sms = 0;
+    int tile_k = 0;
+    long long n_k = 0, n_k_padded = 0, n_tiles = 0;
+    size_t elem = 4;
+    size_t bank_bytes = 0, ws_bytes = 0;
+    size_t ws_xhat = 0, ws_spec = 0, ws_stage_m = 0, ws_stage_h = 0;   // offsets into the workspace
+    void *bank = nullptr, *ws = nullptr;
+    bool own_bank = false, own_ws = false, built = false;
+    void *tw_x = nullptr, *tw_y = nullptr;           // plan precision, 2nx and 2ny entries
+    void *tw_x64 = nullptr, *tw_y64 = nullptr;       // fp64 (setup); alias tw_x/tw_y for an fp64 plan
+    bool profiling = false;
+    int prof_calls = 0;
+    std::vector<cudaEvent_t> prof_events;            // (HFFT_NUM_STAGES + 1) per call
+    std::string error;
+};
+
+static hfft_status fail(hfft_plan* p, hfft_status s, const std::string& msg) {
+    if (p) p->error = msg; else g_create_error = msg;
+    return s;
+}
+static hfft_status fail_cuda(hfft_plan* p, const char* what, cudaError_t e) {
+    return fail(p, HFFT_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+static bool is_pow2(int v) { return v > 0 && (v & (v - 1)) == 0; }
+static int ilog2(int v) { int l = 0; while ((1 << l) < v) ++l; return l; }
+
+// exp(-2 pi i t / N), t in [0, N): the angle is reduced to the first octant in integers so that
+// every entry is the correctly rounded image of an exact rational multiple of pi
+static void twiddle_table(int N, std::vector<double>& re, std::vector<double>& im) {
+    re.resize(N); im.resize(N);
+    const long double pi = 3.14159265358979323846264338327950288L;
+    for (int t = 0; t < N; ++t) {
+        // angle = 2 pi t / N = (pi/4) * (8 t / N); octant o = floor(8t/N), remainder r/N of an octant
+        long long num = 8LL * t;
+        int o = (int)(num / N);
+        long long r = num % N;                     // angle = (o + r/N) * pi/4
+        long double c, s;
+        // within an octant use the smaller of r/N and 1 - r/N
+        bool flip = (o & 1) != 0;
+        long double frac = flip ? (long double)(N - r) / N : (long double)r / N;   // in [0, 1]
+        long double a = frac * (pi / 4);
+        long double ca = cosl(a), sa = sinl(a);
+        if (r == 0) { ca = flip ? sqrtl(0.5L) : 1.0L; sa = flip ? sqrtl(0.5L) : 0.0L; }
+        // base angle of the octant pair: q = o / 2 quarter turns (+ an eighth handled by flip)
+        // angle = q * pi/2 + (flip ? pi/2 - a : a)
+        long double cb = flip ? sa : ca, sb = flip ? ca : sa;   // cos/sin of the in-quadrant angle
+        switch ((o / 2) & 3) {
+            case 0: c = cb; s = sb; break;
+            case 1: c = -sb; s = cb; break;
+            case 2: c = -cb; s = -sb; break;
+            default: c = sb; s = -cb; break;
+        }
+        re[t] = (double)c;
+        im[t] = (double)(-s);
+    }
+}
+
+static cudaError_t upload_twiddles(int N, bool f32, void** out) {
+    std::vector<double> re, im;
+    twiddle_table(N, re, im);
+    cudaError_t e;
+    if (f32) {
+        std::vector<float> h(2 * (size_t)N);
+        for (int t = 0; t < N; ++t) { h[2 * t] = (float)re[t]; h[2 * t + 1] = (float)im[t]; }
+        if ((e = cudaMalloc(out, h.size() * sizeof(float))) != cudaSuccess) return e;
+        return cudaMemcpy(*out, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice);
+    }
+    std::vector<double> h(2 * (size_t)N);
+    for (int t = 0; t < N; ++t) { h[2 * t] = re[t]; h[2 * t + 1] = im[t]; }
+    if ((e = cudaMalloc(out, h.size() * sizeof(double))) != cudaSuccess) return e;
+    return cudaMemcpy(*out, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice);
+}
+
+static void plan_sizes(hfft_plan* p) {
+    const size_t e = p->elem;
+    p->n_k = 2LL * p->ny * (p->nx + 1);
+    // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
+    const int wide = 32 * (int)(16 / e);
+    p->tile_k = (p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148)) ? wide : 32;
+    while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
+    if (p->tile_k != wide) p->tile_k = 32;
+    p->n_tiles = (p->n_k + p->tile_k - 1) / p->tile_k;
+    p->n_k_padded = p->n_tiles * p->tile_k;
+    p->bank_bytes = (size_t)6 * p->nz * p->nz * (size_t)p->n_k_padded * e;
+    const size_t planes = (size_t)3 * p->nz * p->batch;
+    auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    size_t o = 0;
+    p->ws_xhat = o;    o += al(planes * (size_t)p->ny * (p->nx + 1) * 2 * e);
+    p->ws_spec = o;    o += al(planes * (size_t)p->n_k_padded * 2 * e);
+    p->ws_stage_m = o; o += al(planes * (size_t)p->ny * p->nx * e);
+    p->ws_stage_h = o; o += al(planes * (size_t)p->ny * p->nx * e);
+    p->ws_bytes = o;
+}
+
+extern "C" {
+
+const char* hfft_version(void) { return "hfft 0.1 sm_100a"; }
+
+const char* hfft_last_error(const hfft_plan* plan) { return plan ? plan->error.c_str() : g_create_error.c_str(); }
+
+hfft_status hfft_plan_create(hfft_plan** out, int nx, int ny, int nz, double dx, double dy, const double* dz,
+                             hfft_precision precision) {
+    if (!out) return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: out is NULL");
+    *out = nullptr;
+    if (!dz) return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: dz is NULL");
+    if (nx < 2 || ny < 2 || nz < 1) return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: need nx, ny >= 2 and nz >= 1");
+    if (!(dx > 0) || !(dy > 0) || !isfinite(dx) || !isfinite(dy))
+        return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: dx, dy must be positive and finite");
+    for (int k = 0; k < nz; ++k)
+        if (!(dz[k] > 0) || !isfinite(dz[k]))
+            return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: every dz[k] must be positive and finite");
+    if (precision != HFFT_F32 && precision != HFFT_F64)
+        return fail(nullptr, HFFT_EINVAL, "hfft_plan_create: unknown precision");
+    if (!is_pow2(nx) || !is_pow2(ny))
+        return fail(nullptr, HFFT_EUNSUPPORTED, "hfft_plan_create: nx and ny must be powers of two");
+    if (nx > 1024 || ny > 1024) return fail(nullptr, HFFT_EUNSUPPORTED, "hfft_plan_create: nx, ny <= 1024");
+    if (nz > HFFT_MAX_NZ) return fail(nullptr, HFFT_EUNSUPPORTED, "hfft_plan_create: nz exceeds HFFT_MAX_NZ");
+
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return fail_cuda(nullptr, "cudaGetDevice (no CUDA device: this library has no CPU path)", e);
+    cudaDeviceProp prop;
+    if ((e = cudaGetDeviceProperties(&prop, dev)) != cudaSuccess) return fail_cuda(nullptr, "cudaGetDeviceProperties", e);
+    if (prop.major != 10)
+        return fail(nullptr, HFFT_EUNSUPPORTED, "hfft_plan_create: device is not compute capability 10.x (built for sm_100a)");
+
+    hfft_plan* p = new (std::nothrow) hfft_plan();
+    if (!p) return fail(nullptr, HFFT_ENOMEM, "hfft_plan_create: out of host memory");
+    p->nx = nx; p->ny = ny; p->nz = nz; p->dx = dx; p->dy = dy; p->prec = precision;
+    p->log2nx = ilog2(nx); p->log2ny = ilog2(ny);
+    p->dz.assign(dz, dz + nz);
+    p->device = dev; p->num_sms = prop.multiProcessorCount;
+    p->elem = precision == HFFT_F32 ? 4 : 8;
+    plan_sizes(p);
+    if (coupling_smem_bytes(nz, p->tile_k, p->elem) > 200 * 1024) {
+        delete p;
+        return fail(nullptr, HFFT_EUNSUPPORTED, "hfft_plan_create: nz too large for the coupling kernel's shared memory");
+    }
+    *out = p;
+    return HFFT_OK;
+}
+
+hfft_status hfft_plan_set_batch(hfft_plan* plan, int batch) {
+    if (!plan) return HFFT_EINVAL;
+    if (batch < 1) return fail(plan, HFFT_EINVAL, "hfft_plan_set_batch: batch < 1");
+    if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_batch: after build / set_buffers");
+    plan->batch = batch;
+    plan_sizes(plan);
+    return HFFT_OK;
+}
+
+hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
+    if (!plan || !info) return HFFT_EINVAL;
+    info->nx = plan->nx; info->ny = plan->ny; info->nz = plan->nz; info->batch = plan->batch;
+    info->precision = plan->prec; info->tile_k = plan->tile_k;
+    info->n_k = plan->n_k; info->n_k_padded = plan->n_k_padded;
+    info->bank_bytes = plan->bank_bytes; info->workspace_bytes = plan->ws_bytes;
+    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
+                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec};
+    info->setup_scratch_bytes = build_scratch_bytes(g);
+    info->launches_per_demag = HFFT_NUM_STAGES;
+    info->built = plan->built ? 1 : 0;
+    return HFFT_OK;
+}
+
+hfft_status hfft_plan_set_buffers(hfft_plan* plan, void* bank, void* workspace) {
+    if (!plan) return HFFT_EINVAL;
+    if (!bank || !workspace) return fail(plan, HFFT_EINVAL, "hfft_plan_set_buffers: NULL buffer");
+    if (((size_t)bank & 255) || ((size_t)workspace & 255))
+        return fail(plan, HFFT_EINVAL, "hfft_plan_set_buffers: buffers must be 256-byte aligned");
+    if (plan->built) return fail(plan, HFFT_ESTATE, "hfft_plan_set_buffers: after hfft_build_tensor");
+    plan->bank = bank; plan->ws = workspace; plan->own_bank = plan->own_ws = false;
+    return HFFT_OK;
+}
+
+hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    if (!plan->bank) {
+        if ((e = cudaMalloc(&plan->bank, plan->bank_bytes)) != cudaSuccess)
+            return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(bank): ") + cudaGetErrorString(e));
+        plan->own_bank = true;
+    }
+    if (!plan->ws) {
+        if ((e = cudaMalloc(&plan->ws, plan->ws_bytes)) != cudaSuccess)
+            return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(workspace): ") + cudaGetErrorString(e));
+        plan->own_ws = true;
+    }
+    // padded wavevectors of the spectra must hold finite values
+    if ((e = cudaMemsetAsync(plan->ws, 0, plan->ws_bytes, st)) != cudaSuccess) return fail_cuda(plan, "cudaMemsetAsync", e);
+    if (!plan->tw_x64) {
+        if ((e = upload_twiddles(2 * plan->nx, false, &plan->tw_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if ((e = upload_twiddles(2 * plan->ny, false, &plan->tw_y64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if (plan->prec == HFFT_F32) {
+            if ((e = upload_twiddles(2 * plan->nx, true, &plan->tw_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+            if ((e = upload_twiddles(2 * plan->ny, true, &plan->tw_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        } else {
+            plan->tw_x = plan->tw_x64; plan->tw_y = plan->tw_y64;
+        }
+    }
+    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
+                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec};
+    void* scratch = nullptr;
+    const size_t sb = build_scratch_bytes(g);
+    if ((e = cudaMalloc(&scratch, sb)) != cudaSuccess)
+        return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
+    std::string msg;
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->tw_y64, st, msg);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(scratch);
+    if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_build_tensor: " + msg);
+    if (e2 != cudaSuccess) return fail_cuda(plan, "hfft_build_tensor: cudaStreamSynchronize", e2);
+    plan->built = true;
+    return HFFT_OK;
+}
+
+}  // extern "C"
+
+template <typename T>
+static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, void* h, cudaStream_t st) {
+    unsigned char* ws = static_cast<unsigned char*>(p->ws);
+    const int planes = 3 * p->nz * p->batch;
+    const int nrows = planes * p->ny;
+    void* xmain = ws + p->ws_xhat;
+    void* xnyq = ws + p->ws_xhat + (size_t)nrows * p->nx * 2 * sizeof(T);
+    void* spec = ws + p->ws_spec;
+    cudaEvent_t* ev = nullptr;
+    if (p->profiling) {
+        if (p->prof_calls >= kMaxProfileCalls) return fail(p, HFFT_ESTATE, "hfft_demag: profile buffer full; call hfft_profile_read");
+        ev = p->prof_events.data() + (size_t)p->prof_calls * (HFFT_NUM_STAGES + 1);
+    }
+    cudaError_t e;
+#define STAGE(idx, call)                                                            \
+    if (ev && (e = cudaEventRecord(ev[idx], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e); \
+    if ((e = (call)) != cudaSuccess) return fail_cuda(p, #call, e);
+    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xmain, xnyq, p->log2nx, nrows, p->ny, p->nz, Ms, p->tw_x, st)))
+    STAGE(1, (launch_ffty_fwd<T, true>(xmain, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
+    STAGE(2, (launch_coupling<T>(p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded, p->num_sms, st)))
+    STAGE(3, (launch_iffty<T>(spec, xmain, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
+    STAGE(4, (launch_ifftx<T>(xmain, xnyq, (T*)h, p->log2nx, nrows, p->tw_x, st)))
+#undef STAGE
+    if (ev) {
+        if ((e = cudaEventRecord(ev[HFFT_NUM_STAGES], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);
+        p->prof_calls++;
+    }
+    return HFFT_OK;
+}
+
+extern "C" {
+
+hfft_status hfft_demag(hfft_plan* plan, const void* m, const double* Ms, void* h, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (!m || !h) return fail(plan, HFFT_EINVAL, "hfft_demag: NULL m or h");
+    if (((size_t)m & 15) || ((size_t)h & 15)) return fail(plan, HFFT_EINVAL, "hfft_demag: m and h must be 16-byte aligned");
+    if (m == h) return fail(plan, HFFT_EINVAL, "hfft_demag: h must not alias m");
+    if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag: call hfft_build_tensor first");
+    cudaStream_t st = (cudaStream_t)stream;
+    return plan->prec == HFFT_F32 ? demag_impl<float>(plan, m, Ms, h, st) : demag_impl<double>(plan, m, Ms, h, st);
+}
+
+hfft_status hfft_demag_host(hfft_plan* plan, const void* m_host, const double* Ms, void* h_host, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (!m_host || !h_host) return fail(plan, HFFT_EINVAL, "hfft_demag_host: NULL m or h");
+    if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag_host: call hfft_build_tensor first");
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char* ws = static_cast<unsigned char*>(plan->ws);
+    const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
+    cudaError_t e;
+    if ((e = cudaMemcpyAsync(ws + plan->ws_stage_m, m_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return fail_cuda(plan, "cudaMemcpyAsync(H2D)", e);
+    hfft_status s = hfft_demag(plan, ws + plan->ws_stage_m, Ms, ws + plan->ws_stage_h, stream);
+    if (s != HFFT_OK) return s;
+    if ((e = cudaMemcpyAsync(h_host, ws + plan->ws_stage_h, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+        return fail_cuda(plan, "cudaMemcpyAsync(D2H)", e);
+    return HFFT_OK;
+}
+
+hfft_status hfft_profile_enable(hfft_plan* plan, int on) {
+    if (!plan) return HFFT_EINVAL;
+    if (on && plan->prof_events.empty()) {
+        plan->prof_events.resize((size_t)kMaxProfileCalls * (HFFT_NUM_STAGES + 1));
+        for (auto& ev : plan->prof_events) {
+            cudaError_t e = cudaEventCreate(&ev);
+            if (e != cudaSuccess) return fail_cuda(plan, "cudaEventCreate", e);
+        }
+    }
+    plan->profiling = on != 0;
+    plan->prof_calls = 0;
+    return HFFT_OK;
+}
+
+hfft_status hfft_profile_read(hfft_plan* plan, double stage_ms[HFFT_NUM_STAGES], int* calls) {
+    if (!plan || !stage_ms || !calls) return HFFT_EINVAL;
+    for (int s = 0; s < HFFT_NUM_STAGES; ++s) stage_ms[s] = 0.0;
+    *calls = plan->prof_calls;
+    if (plan->prof_calls == 0) return HFFT_OK;
+    cudaError_t e = cudaEventSynchronize(plan->prof_events[(size_t)plan->prof_calls * (HFFT_NUM_STAGES + 1) - 1]);
+    if (e != cudaSuccess) return fail_cuda(plan, "cudaEventSynchronize", e);
+    for (int c = 0; c < plan->prof_calls; ++c) {
+        cudaEvent_t* ev = plan->prof_events.data() + (size_t)c * (HFFT_NUM_STAGES + 1);
+        for (int s = 0; s < HFFT_NUM_STAGES; ++s) {
+            float ms = 0.f;
+            if ((e = cudaEventElapsedTime(&ms, ev[s], ev[s + 1])) != cudaSuccess) return fail_cuda(plan, "cudaEventElapsedTime", e);
+            stage_ms[s] += ms;
+        }
+    }
+    plan->prof_calls = 0;
+    return HFFT_OK;
+}
+
+hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* out_host) {
+    if (!plan || !out_host) return HFFT_EINVAL;
+    hfft_plan* p = const_cast<hfft_plan*>(plan);
+    if (i < 0 || i >= p->nz || j < 0 || j >= p->nz || c < 0 || c > 5) return fail(p, HFFT_EINVAL, "hfft_read_bank: index out of range");
+    if (!p->built) return fail(p, HFFT_ESTATE, "hfft_read_bank: tensor not built");
+    cudaError_t e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return fail_cuda(p, "cudaDeviceSynchronize", e);
+    const int tk = p->tile_k;
+    const double unscale = -4.0 * p->nx * p->ny;
+    std::vector<unsigned char> buf((size_t)tk * p->elem);
+    for (long long t = 0; t < p->n_tiles; ++t) {
+        const size_t off = ((((size_t)t * p->nz + i) * p->nz + j) * 6 + c) * tk * p->elem;
+        e = cudaMemcpy(buf.data(), static_cast<unsigned char*>(p->bank) + off, (size_t)tk * p->elem, cudaMemcpyDeviceToHost);
+        if (e != cudaSuccess) return fail_cuda(p, "cudaMemcpy(bank)", e);
+        for (int kk = 0; kk < tk; ++kk) {
+            long long k = t * tk + kk;
+            if (k >= p->n_k) break;
+            double v = p->elem == 4 ? (double)reinterpret_cast<float*>(buf.data())[kk] : reinterpret_cast<double*>(buf.data())[kk];
+            out_host[k] = v * unscale;
+        }
+    }
+    return HFFT_OK;
+}
+
+hfft_status hfft_destroy(hfft_plan* plan) {
+    if (!plan) return HFFT_OK;
+    if (plan->own_bank && plan->bank) cudaFree(plan->bank);
+    if (plan->own_ws && plan->ws) cudaFree(plan->ws);
+    if (plan->tw_x && plan->tw_x != plan->tw_x64) cudaFree(plan->tw_x);
+    if (plan->tw_y && plan->tw_y != plan->tw_y64) cudaFree(plan->tw_y);
+    if (plan->tw_x64) cudaFree(plan->tw_x64);
+    if (plan->tw_y64) cudaFree(plan->tw_y64);
+    for (auto& ev : plan->prof_events) cudaEventDestroy(ev);
+    delete plan;
+    return HFFT_OK;
+}
+
+}  // extern "C"

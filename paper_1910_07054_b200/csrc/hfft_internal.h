@@ -1,0 +1,54 @@
+// hfft_internal.h -- declarations shared by the translation units of libhfft (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+#include <string>
+#include <vector>
+
+#include "../../include/hfft.h"
+
+namespace hfft {
+
+// per-layer saturation magnetisation, passed by value to the S1 kernel (hfft.h: "read during the
+// call and passed by value to the kernels")
+template <typename T> struct MsParam { T v[HFFT_MAX_NZ]; };
+
+// ---- fft_kernels.cu ----
+// forward x: `in` real rows (nx reals if ZP, 2nx if not) -> main [nrows][nx] + Nyquist [nrows]
+template <typename T, bool ZP>
+cudaError_t launch_fftx_fwd(const T* in, void* out_main, void* out_nyq, int log2nx, int nrows, int rows_per_plane,
+                            int nz, const double* ms_host, const void* tw2nx, cudaStream_t st);
+template <typename T>
+cudaError_t launch_ifftx(const void* in_main, const void* in_nyq, T* out, int log2nx, int nrows, const void* tw2nx,
+                         cudaStream_t st);
+// forward y: row side (main [nplanes*rows][nx] + Nyquist [nplanes*rows]) -> k side [nplanes][ks];
+// nz_rot > 0 multiplies the z-component planes by i
+template <typename T, bool ZP>
+cudaError_t launch_ffty_fwd(const void* in, void* out, int nx, int log2N, int nplanes, int nz_rot, long long ks,
+                            const void* twN, cudaStream_t st);
+template <typename T>
+cudaError_t launch_iffty(const void* in, void* out, int nx, int log2N, int nplanes, int nz_rot, long long ks,
+                         const void* twN, cudaStream_t st);
+
+// ---- coupling.cu ----
+// H^ = bank * M^ in place on the k side.  bank layout [tile][i][j][6][tile_k].
+template <typename T>
+cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
+                            long long ks, int num_sms, cudaStream_t st);
+size_t coupling_smem_bytes(int nz, int tile_k, size_t elem);
+
+// ---- tensor_build.cu ----
+struct BuildGeom {
+    int nx, ny, nz, log2nx, log2ny;
+    double dx, dy;
+    const double* dz;      // host
+    int tile_k;
+    long long n_k, n_k_padded;
+    int prec;              // hfft_precision
+};
+size_t build_scratch_bytes(const BuildGeom& g);
+// fills `bank` (plan precision); tw2nx_f64 / tw2ny_f64 are fp64 twiddle tables on device
+cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx_f64, const void* tw2ny_f64,
+                       cudaStream_t st, std::string& err);
+
+}  // namespace hfft

@@ -1,0 +1,236 @@
+// tensor_build.cu -- stage S0 (timed setup): the spectral tensor bank F1F2(N_kl)_{i3-j3} of Eq.24
+// (PAPER.md:177-178), built on the device.
+//
+// Tensor (PAPER.md:52 Eq.5, :99 Eq.11 with the 4th term read as Y+dy [A1], :249-291 Eq.27-31).
+// Multiplying out Eq.5 x Eq.28 x Eq.27 (F2 -> f) and Eq.11 x Eq.31 x Eq.30
+// (G2 -> g) gives, for all six components c with their permuted primitive phi_c
+// (newell_dd.cuh), one signed 4 x 4 x 4 stencil.  In the plane target and source cells have the
+// same size, so the x and y stencils collapse to second differences; along z the four points are
+// the interface differences of the two layers (Z_ij = zeta_i - zeta_j, lower faces, reading A8):
+//
+//   Psi_c(a, b)(p, q) = sum_{al,be in {-1,0,1}} w_al w_be phi_c((p+al) dx, (q+be) dy, zeta_a - zeta_b),
+//                       w = (1, -2, 1)
+//   N^c_ij(p dx, q dy) = -1 / (4 pi dx dy dz_i) [ Psi_c(i+1, j) - Psi_c(i, j) - Psi_c(i+1, j+1) + Psi_c(i, j+1) ]
+//
+// with |tau| = dx dy dz_i the TARGET volume (reading A7).  Everything up to the
+// rounding of N to fp64 runs in double-double (reading A16).
+//
+// Then: N is laid on the 2nx x 2ny periodic grid at (p mod 2nx, q mod 2ny), the slots p = nx and
+// q = ny are 0 (reading A10), negative offsets come from the parities of the components (xx, yy,
+// zz even in X and Y; xy odd, odd; xz odd, even; yz even, odd); a full (not zero-padded) fp64
+// real-to-complex 2-D FFT follows, and the real part (xx, yy, zz, xy) or imaginary part (xz, yz)
+// times -1/(4 nx ny) is stored in the plan precision at bank[tile][i][j][c][k in tile].
+#include "hfft_internal.h"
+#include "newell_dd.cuh"
+
+namespace hfft {
+
+__constant__ int kParX[6] = {+1, +1, +1, -1, -1, +1};
+__constant__ int kParY[6] = {+1, +1, +1, -1, +1, -1};
+__constant__ int kParZ[6] = {+1, +1, +1, +1, -1, -1};
+
+// phi[b][c][Q][P], Q in [0, ny], P in [0, nx], z = zeta[a] - zeta[b]
+__global__ void __launch_bounds__(128)
+lattice_kernel(double2* __restrict__ phi, const double2* __restrict__ zeta, int a, int nx, int ny, int nz,
+               double dx, double dy) {
+    const int P = blockIdx.x * blockDim.x + threadIdx.x;
+    const int Q = blockIdx.y;
+    const int b = blockIdx.z;
+    if (P > nx) return;
+    dd za = dd_make(zeta[a].x, zeta[a].y), zb = dd_make(zeta[b].x, zeta[b].y);
+    dd z = dd_sub(za, zb);
+    const bool zneg = z.hi < 0.0;
+    z = dd_abs(z);
+    dd x = two_prod((double)P, dx), y = two_prod((double)Q, dy);
+    dd v[6];
+    newell_phi6(x, y, z, v);
+    const size_t plane = (size_t)(ny + 1) * (nx + 1);
+    size_t o = (size_t)b * 6 * plane + (size_t)Q * (nx + 1) + P;
+#pragma unroll
+    for (int c = 0; c < 6; ++c) {
+        dd u = (zneg && kParZ[c] < 0) ? dd_neg(v[c]) : v[c];
+        phi[o + c * plane] = make_double2(u.hi, u.lo);
+    }
+}
+
+// psi[b][c][q][p] = second difference in x and in y of phi, p in [0, nx), q in [0, ny)
+__global__ void __launch_bounds__(128)
+stencil_kernel(double2* __restrict__ psi, const double2* __restrict__ phi, int nx, int ny) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int q = blockIdx.y;
+    const int bc = blockIdx.z;          // b * 6 + c
+    if (p >= nx) return;
+    const int c = bc % 6;
+    const double2* f = phi + (size_t)bc * (ny + 1) * (nx + 1);
+    dd acc = dd_make(0.0, 0.0);
+#pragma unroll
+    for (int be = -1; be <= 1; ++be) {
+        int Q = q + be;
+        double sy = 1.0;
+        if (Q < 0) { Q = -Q; sy = (double)kParY[c]; }
+        dd row = dd_make(0.0, 0.0);
+#pragma unroll
+        for (int al = -1; al <= 1; ++al) {
+            int P = p + al;
+            double sx = 1.0;
+            if (P < 0) { P = -P; sx = (double)kParX[c]; }
+            double2 t = f[(size_t)Q * (nx + 1) + P];
+            double w = (al == 0 ? -2.0 : 1.0) * sx;
+            row = dd_add(row, dd_make(t.x * w, t.y * w));
+        }
+        double w = (be == 0 ? -2.0 : 1.0) * sy;
+        acc = dd_add(acc, dd_make(row.hi * w, row.lo * w));
+    }
+    psi[((size_t)bc * ny + q) * nx + p] = make_double2(acc.hi, acc.lo);
+}
+
+// N^c_ij on the padded periodic grid: R[jl][c][2ny][2nx] (fp64), jl = j - j0
+__global__ void __launch_bounds__(128)
+assemble_kernel(double* __restrict__ R, const double2* __restrict__ psi_lo /* a = i */,
+                const double2* __restrict__ psi_hi /* a = i+1 */, int nx, int ny, int j0, double2 neg_inv_4pi_tau) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    const int q = blockIdx.y;
+    const int jc = blockIdx.z;          // jl * 6 + c
+    if (p >= nx) return;
+    const int jl = jc / 6, c = jc - jl * 6;
+    const int j = j0 + jl;
+    const size_t pl = (size_t)ny * nx;
+    const size_t o = (size_t)q * nx + p;
+    auto ld = [&](const double2* s, int b) {
+        double2 t = s[((size_t)b * 6 + c) * pl + o];
+        return dd_make(t.x, t.y);
+    };
+    dd s = dd_sub(ld(psi_hi, j), ld(psi_lo, j));
+    s = dd_sub(s, ld(psi_hi, j + 1));
+    s = dd_add(s, ld(psi_lo, j + 1));
+    s = dd_mul(s, dd_make(neg_inv_4pi_tau.x, neg_inv_4pi_tau.y));
+    const double v = s.hi;
+    const double sx = (double)kParX[c], sy = (double)kParY[c];
+    double* dst = R + (size_t)jc * 4 * pl;
+    const int W = 2 * nx, H = 2 * ny;
+    dst[(size_t)q * W + p] = v;
+    if (p > 0) dst[(size_t)q * W + (W - p)] = v * sx;
+    if (q > 0) dst[(size_t)(H - q) * W + p] = v * sy;
+    if (p > 0 && q > 0) dst[(size_t)(H - q) * W + (W - p)] = v * sx * sy;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(256)
+pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, int j0, int jcount, int tile_k,
+            long long n_k, long long n_k_padded, double scale) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int jc = blockIdx.y;          // jl * 6 + c
+    if (k >= n_k_padded) return;
+    const int jl = jc / 6, c = jc - jl * 6;
+    double v = 0.0;
+    if (k < n_k) {
+        double2 t = Y[(size_t)jc * n_k + k];
+        v = (c < 4 ? t.x : t.y) * scale;
+    }
+    const long long tile = k / tile_k;
+    const int kk = (int)(k - tile * tile_k);
+    bank[(((tile * nz + i) * nz + (j0 + jl)) * 6 + c) * tile_k + kk] = (T)v;
+    (void)jcount;
+}
+
+struct ScratchLayout {
+    size_t zeta, phi, psi0, psi1, R, X, Y, total;
+    int jc;
+};
+
+static ScratchLayout scratch_layout(const BuildGeom& g) {
+    ScratchLayout L;
+    auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
+    const size_t nxy = (size_t)g.nx * g.ny;
+    const size_t per_j = 6 * (4 * nxy * 8 + 2 * (size_t)g.n_k * 16);
+    size_t jc = ((size_t)1 << 30) / per_j;
+    if (jc < 1) jc = 1;
+    if (jc > (size_t)g.nz) jc = g.nz;
+    L.jc = (int)jc;
+    size_t o = 0;
+    L.zeta = o; o += al((size_t)(g.nz + 1) * 16);
+    L.phi = o;  o += al((size_t)(g.nz + 1) * 6 * (g.ny + 1) * (g.nx + 1) * 16);
+    L.psi0 = o; o += al((size_t)(g.nz + 1) * 6 * nxy * 16);
+    L.psi1 = o; o += al((size_t)(g.nz + 1) * 6 * nxy * 16);
+    L.R = o;    o += al(jc * 6 * 4 * nxy * 8);
+    L.X = o;    o += al(jc * 6 * (size_t)g.n_k * 16);
+    L.Y = o;    o += al(jc * 6 * (size_t)g.n_k * 16);
+    L.total = o;
+    return L;
+}
+
+size_t build_scratch_bytes(const BuildGeom& g) { return scratch_layout(g).total; }
+
+#define HFFT_CK(call)                                                                  \
+    do {                                                                               \
+        cudaError_t e_ = (call);                                                       \
+        if (e_ != cudaSuccess) {                                                       \
+            err = std::string(#call) + ": " + cudaGetErrorString(e_);                  \
+            return e_;                                                                 \
+        }                                                                              \
+    } while (0)
+
+cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx, const void* tw2ny,
+                       cudaStream_t st, std::string& err) {
+    const ScratchLayout L = scratch_layout(g);
+    unsigned char* base = static_cast<unsigned char*>(scratch);
+    double2* d_zeta = reinterpret_cast<double2*>(base + L.zeta);
+    double2* d_phi = reinterpret_cast<double2*>(base + L.phi);
+    double2* d_psi[2] = {reinterpret_cast<double2*>(base + L.psi0), reinterpret_cast<double2*>(base + L.psi1)};
+    double* d_R = reinterpret_cast<double*>(base + L.R);
+    double2* d_X = reinterpret_cast<double2*>(base + L.X);
+    double2* d_Y = reinterpret_cast<double2*>(base + L.Y);
+    const int nx = g.nx, ny = g.ny, nz = g.nz;
+
+    // lower-face coordinates zeta_0 = 0, zeta_{k+1} = zeta_k + dz_k in double-double (reading A8/A9)
+    std::vector<double2> zeta(nz + 1);
+    dd acc = dd_make(0.0, 0.0);
+    zeta[0] = make_double2(0.0, 0.0);
+    for (int k = 0; k < nz; ++k) {
+        acc = dd_add_d(acc, g.dz[k]);
+        zeta[k + 1] = make_double2(acc.hi, acc.lo);
+    }
+    HFFT_CK(cudaMemcpyAsync(d_zeta, zeta.data(), sizeof(double2) * (nz + 1), cudaMemcpyHostToDevice, st));
+    HFFT_CK(cudaStreamSynchronize(st));   // `zeta` is pageable host memory
+    HFFT_CK(cudaMemsetAsync(d_R, 0, (size_t)L.jc * 6 * 4 * nx * ny * 8, st));   // slots p = nx, q = ny stay 0
+
+    const double scale = -1.0 / (4.0 * (double)nx * (double)ny);
+    const dd inv4pi = dd_make(DD_INV_4PI_HI, DD_INV_4PI_LO);
+    for (int a = 0; a <= nz; ++a) {
+        {
+            dim3 grid((nx + 1 + 127) / 128, ny + 1, nz + 1);
+            lattice_kernel<<<grid, 128, 0, st>>>(d_phi, d_zeta, a, nx, ny, nz, g.dx, g.dy);
+            HFFT_CK(cudaGetLastError());
+            dim3 grid2((nx + 127) / 128, ny, (nz + 1) * 6);
+            stencil_kernel<<<grid2, 128, 0, st>>>(d_psi[a & 1], d_phi, nx, ny);
+            HFFT_CK(cudaGetLastError());
+        }
+        if (a == 0) continue;
+        const int i = a - 1;
+        // -1 / (4 pi dx dy dz_i) in double-double
+        dd tau = dd_mul_d(two_prod(g.dx, g.dy), g.dz[i]);
+        dd coef = dd_neg(dd_div(inv4pi, tau));
+        for (int j0 = 0; j0 < nz; j0 += L.jc) {
+            const int jn = (nz - j0 < L.jc) ? nz - j0 : L.jc;
+            dim3 grid((nx + 127) / 128, ny, jn * 6);
+            assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
+                                                  make_double2(coef.hi, coef.lo));
+            HFFT_CK(cudaGetLastError());
+            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, d_X + (size_t)jn * 6 * 2 * ny * nx, g.log2nx,
+                                                    jn * 6 * 2 * ny, 2 * ny, 0, nullptr, tw2nx, st)));
+            HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, tw2ny, st)));
+            dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
+            if (g.prec == HFFT_F32)
+                pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, jn, g.tile_k, g.n_k,
+                                                          g.n_k_padded, scale);
+            else
+                pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, jn, g.tile_k, g.n_k,
+                                                           g.n_k_padded, scale);
+            HFFT_CK(cudaGetLastError());
+        }
+    }
+    HFFT_CK(cudaStreamSynchronize(st));
+    return cudaSuccess;
+}
+
+}  // namespace hfft

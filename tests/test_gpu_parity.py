@@ -1,0 +1,190 @@
+"""Parity of the CUDA path (through the C ABI, include/hfft.h) with the CPU oracle.  -m gpu.
+
+Tolerances are BASELINE.json's: max|H_gpu - H_ref| / max|H_ref| <= 1e-12 (fp64), <= 2e-6 (fp32).
+The oracle gets the inputs rounded to the plan precision and promoted back to fp64, so input
+rounding is not charged to the GPU path.
+"""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1910_07054_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f32": 2e-6, "f64": 1e-12}
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    from paper_1910_07054_b200 import binding
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    binding.lib()   # fails loudly if libhfft.so is missing
+    return binding
+
+
+def _relerr(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _run(hb, w, m=None, Ms="w", host=False):
+    """m: fp64 [B][3][nz][ny][nx] already rounded to the plan precision."""
+    import torch
+    if m is None:
+        m = w.m_rounded()
+    if isinstance(Ms, str):
+        Ms = w.Ms
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=m.shape[0])
+    plan.build_tensor()
+    dt = torch.float32 if w.precision == "f32" else torch.float64
+    if host:
+        mh = torch.from_numpy(m).to(dt).pin_memory()
+        hh = plan.demag_host(mh, Ms)
+        torch.cuda.synchronize()
+        H = hh.double().numpy().copy()
+    else:
+        md = torch.from_numpy(m).to(dt).cuda()
+        h = plan.demag(md, Ms)
+        torch.cuda.synchronize()
+        H = h.double().cpu().numpy()
+    return plan, H
+
+
+def _oracle_nhat(w, i):
+    """In-plane DFT of the oracle's tensor row i in the library's k order: [nz][6][n_k] complex."""
+    nx, ny = w.nx, w.ny
+    row = O.tensor_row(nx, ny, w.nz, w.dx, w.dy, w.dz, i)
+    pad = np.zeros((w.nz, 6, 2 * ny, 2 * nx))
+    p = np.arange(-(nx - 1), nx)
+    q = np.arange(-(ny - 1), ny)
+    pad[:, :, (q % (2 * ny))[:, None], (p % (2 * nx))[None, :]] = row
+    Nh = np.fft.fft2(pad, axes=(-2, -1))
+    main = Nh[..., :, :nx].reshape(w.nz, 6, -1)
+    nyq = Nh[..., :, nx]
+    return np.concatenate([main, nyq], axis=-1)
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_bank_matches_oracle_spectrum(hb, prec):
+    """S0: every plane of the device-built bank against the oracle tensor's numpy FFT, including
+    the purity R5 (xx,yy,zz,xy real; xz,yz imaginary) that the real storage relies on."""
+    w = W.small(8, 16, 3, precision=prec, seed=11)
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec)
+    plan.build_tensor()
+    tol = 1e-13 if prec == "f64" else 3e-7
+    for i in range(w.nz):
+        ref = _oracle_nhat(w, i)
+        scale = np.abs(ref).max()
+        assert np.abs(ref[:, :4].imag).max() < 1e-14 * scale
+        assert np.abs(ref[:, 4:].real).max() < 1e-14 * scale
+        for j in range(w.nz):
+            for c in range(6):
+                got = hb.read_bank(plan.handle, i, j, c)
+                want = ref[j, c].real if c < 4 else ref[j, c].imag
+                assert np.abs(got - want).max() <= tol * scale, (i, j, c)
+    plan.close()
+
+
+def test_config1_full_grid_fp64_vs_direct_sum(hb):
+    """C1 (16 x 16 x 3, fp64): every cell against the O(n^2) direct real-space sum (T0, Eq.18)."""
+    w = W.config(1)
+    plan, H = _run(hb, w)
+    ref = O.direct_field(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.m_rounded()[0], w.Ms)
+    assert H.shape == (1, 3, w.nz, w.ny, w.nx)
+    assert _relerr(H[0], ref) <= TOL["f64"]
+    plan.close()
+
+
+@pytest.mark.parametrize("variant", ["f64", ""])
+def test_config2_mram_stack(hb, variant):
+    """C2 (64 x 64 x 6, per-layer Ms, fp32 and fp64) against the hybrid oracle (T1) on every cell
+    and against the direct sum (T0) on sampled cells."""
+    w = W.config(2, variant)
+    m = w.m_rounded()
+    plan, H = _run(hb, w, m)
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m[0], w.Ms, dft="fft")
+    assert _relerr(H[0], ref) <= TOL[w.precision]
+    rng = np.random.default_rng(7)
+    for i in (0, 5):
+        cells = rng.choice(w.nx * w.ny, size=200, replace=False).astype(np.int32)
+        H0 = O.direct_cells(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m[0], w.Ms, i, cells)
+        got = H[0][:, i].reshape(3, -1)[:, cells].T
+        assert np.abs(got - H0).max() / np.abs(ref).max() <= TOL[w.precision]
+    plan.close()
+
+
+SHAPES = [
+    # nx, ny, nz, B   -- ragged (nx != ny), tiny, single layer, odd layer counts, several tiles + tail
+    (2, 2, 1, 1), (2, 4, 2, 1), (4, 2, 3, 2), (8, 32, 5, 1), (32, 8, 1, 3), (16, 16, 7, 2), (64, 32, 4, 1),
+    (128, 16, 2, 1), (32, 128, 3, 1),
+]
+
+
+@pytest.mark.parametrize("nx,ny,nz,B", SHAPES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_small_shapes_vs_hybrid_oracle(hb, nx, ny, nz, B, prec):
+    w = W.small(nx, ny, nz, precision=prec, B=B, seed=100 + nx + 3 * ny + 7 * nz)
+    m = w.m_rounded()
+    plan, H = _run(hb, w, m)
+    ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    if nx * ny * nz <= 2048:
+        ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, w.dz, m[0], w.Ms)
+        assert _relerr(H[0], ref0) <= TOL[prec]
+    plan.close()
+
+
+def test_ms_null_scalar_and_host_path(hb):
+    """Ms = NULL means m already holds M (hfft.h); the host-buffer entry point gives the same field."""
+    w = W.small(16, 8, 3, precision="f64", seed=5)
+    m = w.m_rounded()
+    M = m * w.Ms[None, None, :, None, None]
+    plan, H1 = _run(hb, w, m)
+    _, H2 = _run(hb, w, M, Ms=None)
+    _, H3 = _run(hb, w, m, host=True)
+    assert _relerr(H2, H1) < 1e-14
+    assert np.array_equal(H3, H1)
+    plan.close()
+
+
+def test_uniform_cube_gives_one_third(hb):
+    """Closed form: a uniformly magnetised cube has <H> = -Ms/3 per axis."""
+    import torch
+    n, nz = 8, 4
+    dz = np.array([1.0, 3.0, 2.5, 1.5])      # sums to 8 = n * dx
+    plan = hb.Plan(n, n, nz, 1.0, 1.0, dz, "f64")
+    plan.build_tensor()
+    for a in range(3):
+        m = torch.zeros((1, 3, nz, n, n), dtype=torch.float64, device="cuda")
+        m[0, a] = 1.0
+        H = plan.demag(m, 8e5).cpu().numpy()[0]
+        avg = (H * dz[None, :, None, None]).sum(axis=(1, 2, 3)) / (n * n * dz.sum())
+        want = np.zeros(3)
+        want[a] = -8e5 / 3
+        assert np.abs(avg - want).max() < 1e-9 * 8e5
+    plan.close()
+
+
+def test_argument_errors(hb):
+    dz = np.array([1.0, 2.0])
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_create(12, 16, 2, 1.0, 1.0, dz, hb.F32)
+    assert e.value.status == hb.EUNSUPPORTED
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_create(16, 16, 2, -1.0, 1.0, dz, hb.F32)
+    assert e.value.status == hb.EINVAL
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_create(16, 16, 2, 1.0, 1.0, np.array([1.0, 0.0]), hb.F32)
+    assert e.value.status == hb.EINVAL
+    p = hb.plan_create(16, 16, 2, 1.0, 1.0, dz, hb.F32)
+    import torch
+    x = torch.zeros(3 * 2 * 16 * 16, device="cuda")
+    with pytest.raises(hb.HfftError) as e:       # demag before build_tensor
+        hb.demag(p, x.data_ptr(), None, x.data_ptr() + 0, 0)
+    assert e.value.status in (hb.ESTATE, hb.EINVAL)
+    y = torch.zeros_like(x)
+    with pytest.raises(hb.HfftError) as e:
+        hb.demag(p, x.data_ptr(), None, y.data_ptr(), 0)
+    assert e.value.status == hb.ESTATE
+    hb.destroy(p)
