@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- demagnetization-field evaluations per second of hfft_demag on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+A "step" is one pass of the whole hot path (S1 x-FFT, S2 y-FFT, S3 layer coupling, S4 inverse
+y-FFT, S5 inverse x-FFT) over one batch of synthetic magnetisation, i.e. one
+hfft_demag call (B field evaluations; B = 1 except config 5).  Default workload: BASELINE.json
+configs[3], the 256 x 256 x 64 non-equidistant fp32 stack that north_star's target is quoted on
+(tensor bank 12.9 GB, far larger than L2, so every step streams it from HBM).
+
+Prints ONE JSON line (contract in the task statement).  Multi-GPU: the method does not shard
+(north_star: one GPU, no collectives) -- N ranks run N independent replicas ("replicas only").
+`--impl reference` times the CPU oracle (oracle/, T1 hybrid with numpy FFT) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_1910_07054_b200 import workloads as W  # noqa: E402
+
+METRIC = "demag_field_evals_per_sec"
+UNIT = "evals/s"
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", default="4", help="BASELINE.json config 1..5, '2f64', '4eq'")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def get_workload(name):
+    if name == "2f64":
+        return W.config(2, "f64")
+    if name == "4eq":
+        return W.config(4, "equal")
+    return W.config(int(name))
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as fh:
+            d = json.load(fh)
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def algorithmic_bytes(w):
+    """what the shipped storage must move per hfft_demag call."""
+    s = 4 if w.precision == "f32" else 8
+    n_k = 2 * w.ny * (w.nx + 1)
+    planes = 3 * w.nz * w.B
+    bank = 6 * w.nz * w.nz * n_k * s
+    spec = planes * n_k * 2 * s            # M^ (= H^)
+    xhat = planes * w.ny * (w.nx + 1) * 2 * s
+    field = planes * w.ny * w.nx * s
+    coupling = bank + 2 * spec
+    whole = 2 * field + 4 * xhat + 4 * spec + bank
+    return {"bank": bank, "coupling": coupling, "whole": whole}
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+
+    def __init__(self, index):
+        self.index = index
+        self.proc = None
+        self.out = None
+
+    def start(self):
+        self.out = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
+                 "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.out, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return res
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        self.out.flush()
+        self.out.seek(0)
+        sm, mx, reasons = [], [], set()
+        for ln in self.out:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, val in zip(self.NAMES, f[3:7]):
+                if val == "Active":
+                    reasons.add(name)
+        self.out.close()
+        os.unlink(self.out.name)
+        if sm:
+            res.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
+                       samples=len(sm))
+        return res
+
+
+def cpu_baseline(w, budget_s=20.0):
+    """The oracle's hybrid tier (T1, numpy FFT) on target layer 0 of the workload, tensor row
+    prebuilt (setup, like hfft_build_tensor for the GPU).  evals/s = 1 / (nz * t_layer)."""
+    import oracle as O
+    m = w.m_rounded([0])[0]
+    t0 = time.perf_counter()
+    row = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
+    setup = time.perf_counter() - t0
+    times = []
+    while len(times) < 3 or (sum(times) < budget_s and len(times) < 20):
+        t0 = time.perf_counter()
+        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, [0], dft="fft", rows={0: row})
+        times.append(time.perf_counter() - t0)
+        if sum(times) > 4 * budget_s:
+            break
+    t_layer = float(np.median(times))
+    return {"value": 1.0 / (w.nz * t_layer), "unit": UNIT, "cores": O.threads(), "kind": "oracle",
+            "sample": "target layer 0 of %d, one state (oracle.hybrid_layers, numpy FFT, fp64), tensor row "
+                      "prebuilt; median of %d runs of %.3f s; value = 1/(nz*t_layer); numpy's FFT and einsum "
+                      "run on 1 thread, the binary128 tensor row (setup, %.1f s) on `cores` OpenMP threads"
+                      % (w.nz, len(times), t_layer, setup),
+            "oracle_tensor_row_s": setup}
+
+
+def run_reference(args, w):
+    """--impl reference: the oracle, as it stands, on the host cores.  One step = target layer 0."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle as O
+    m = w.m_rounded([0])[0]
+    row = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
+    rows = {0: row}
+
+    def step():
+        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, [0], dft="fft", rows=rows)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = time.perf_counter() - t0
+    t_layer = dt / args.steps
+    value = 1.0 / (w.nz * t_layer) * w.B / w.B      # one state; evals/s of a whole-stack evaluation
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_layer, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, "host memory; no GPU"),
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.threads(), "kind": "oracle",
+                         "sample": "each step = target layer 0 of %d of one state (oracle.hybrid_layers, numpy "
+                                   "FFT, fp64, tensor row prebuilt); value = 1/(nz * s_per_step)" % w.nz},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+
+
+def workload_config(w, l2):
+    return {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "batch": w.B, "precision": w.precision,
+            "dz_nm": [round(float(v), 6) for v in w.dz[:8]] + (["..."] if w.nz > 8 else []),
+            "m": w.m_kind, "seed": w.seed, "l2": l2, "parallelism": "replicas only (no sharding, no collective)"}
+
+
+def main():
+    args = parse_args()
+    w = get_workload(args.config)
+    if args.impl == "reference":
+        run_reference(args, w)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_1910_07054_b200 import binding as hb
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: hfft has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    steps, warmup = max(1, args.steps), max(3, args.warmup)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B)
+    t0 = time.perf_counter()
+    plan.build_tensor()
+    torch.cuda.synchronize()
+    setup_s = time.perf_counter() - t0
+
+    dt = torch.float32 if w.precision == "f32" else torch.float64
+    m_host = torch.from_numpy(w.m_rounded()).to(dt).pin_memory()
+    m = m_host.cuda()
+    h = torch.empty_like(m)
+    h_host = torch.empty_like(m_host).pin_memory()
+    Ms = w.Ms
+    nbytes = m.numel() * m.element_size()
+    ab = algorithmic_bytes(w)
+    # inputs larger than L2?  otherwise flush L2 between steps (and say so)
+    flush = None
+    if ab["whole"] < 512 << 20:
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        if flush is not None:
+            flush.zero_()
+        plan.demag(m, Ms, h)
+
+    for _ in range(warmup):
+        step()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # ---- timed region 1: device-resident inputs ----
+    if flush is None:
+        ev0.record()
+        for _ in range(steps):
+            step()
+        ev1.record()
+        torch.cuda.synchronize()
+        ms_total = ev0.elapsed_time(ev1)
+    else:   # time each step alone so that the flush is outside the timed intervals
+        ms_total = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            ev0.record()
+            plan.demag(m, Ms, h)
+            ev1.record()
+            torch.cuda.synchronize()
+            ms_total += ev0.elapsed_time(ev1)
+    barrier()
+    # ---- timed region 2: same steps with per-stage CUDA events (hfft_profile_*) ----
+    hb.profile_enable(plan.handle, True)
+    stage_ms = np.zeros(hb.NUM_STAGES)
+    calls = 0
+    done = 0
+    while done < steps:
+        n = min(200, steps - done)
+        for _ in range(n):
+            step()
+        ms, c = hb.profile_read(plan.handle)
+        stage_ms += ms
+        calls += c
+        done += n
+    hb.profile_enable(plan.handle, False)
+    stage_ms /= max(calls, 1)
+    # ---- timed region 3: end to end through hfft_demag_host (pinned host buffers) ----
+    for _ in range(3):
+        plan.demag_host(m_host, Ms, h_host)
+    barrier()
+    e2e_steps = max(1, min(steps, 50))
+    ev0.record()
+    for _ in range(e2e_steps):
+        plan.demag_host(m_host, Ms, h_host)
+    ev1.record()
+    torch.cuda.synchronize()
+    ms_e2e = ev0.elapsed_time(ev1)
+    barrier()
+    clocks = sampler.stop()
+
+    assert bool(torch.isfinite(h).all()) and bool(torch.isfinite(h_host).all())
+    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total, ms_e2e = float(t[0]), float(t[1])
+
+    if rank == 0:
+        peak, peak_src = measured_peaks()
+        ms_step = ms_total / steps
+        value = world * w.B * steps / (ms_total * 1e-3)
+        coup_ms = float(stage_ms[hb.STAGE_NAMES.index("coupling")])
+        achieved = ab["coupling"] / (coup_ms * 1e-3) / 1e9 if coup_ms > 0 else None
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            with open(tp) as fh:
+                traffic = json.load(fh).get(w.name, {}).get("coupling_dram_bytes_per_launch")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": w.precision, "data": "synthetic",
+            "config": workload_config(
+                w, "inputs larger than L2 (tensor bank %.2f GB streamed every step)" % (ab["bank"] / 1e9)
+                if flush is None else "L2 flushed (256 MiB memset) before every timed step"),
+            "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
+                       "samples": clocks["samples"]},
+            "e2e": {"value": world * w.B * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
+                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
+                    "api": "hfft_demag_host (pinned host m -> device, 5 kernels, device h -> pinned host)"},
+            "gpu_launches": plan.info.launches_per_demag * steps,
+            "roofline": {"bound": "hbm", "kernel": "coupling_kernel (S3)", "achieved": achieved, "peak": peak,
+                         "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak if achieved else None,
+                         "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None,
+                         "algorithmic_bytes_per_launch": ab["coupling"], "avg_launch_ms": coup_ms,
+                         "traffic": traffic},
+            "stages_ms": {n: float(v) for n, v in zip(hb.STAGE_NAMES, stage_ms)},
+            "whole_eval": {"algorithmic_bytes": ab["whole"], "roofline_ms_at_peak": ab["whole"] / peak / 1e6,
+                           "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
+            "setup_s": setup_s,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline(w)
+        print(json.dumps(line))
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -199,7 +199,7 @@ def _pad_kernel(Nrow, nx, ny):
     return pad
 
 
-def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive"):
+def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive", rows=None):
     """T1: Eq.24 for the listed target layers.
 
       H_{k,i1,i2,i3} = - sum_l F2^-1 F1^-1 sum_{j3} [ F1F2(N_kl)_{i3-j3} F1F2(M_l)_{j3} ]_{i1,i2}
@@ -207,6 +207,8 @@ def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive"):
     with the in-plane transforms taken on the zero-padded 2nx x 2ny grid (A10)
     and the z-sum written out.  m: [3][nz][ny][nx] or [B][3][nz][ny][nx].
     Returns [len(layers)][3][ny][nx] (or [B][len(layers)][3][ny][nx]).
+    rows: optional {i: tensor_row(..., i)} of precomputed tensor rows (setup hoisted out, e.g. when
+    bench.py times the evaluation without the tensor build); the arithmetic is unchanged.
     """
     M = _magnetisation(m, Ms, nz)
     batched = M.ndim == 5
@@ -224,7 +226,9 @@ def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive"):
         raise ValueError(dft)
     out = np.empty((B, len(layers), 3, ny, nx))
     for t, i in enumerate(layers):
-        pad = _pad_kernel(tensor_row(nx, ny, nz, dx, dy, dz, i), nx, ny)
+        Nrow = rows[i] if rows is not None and i in rows else tensor_row(nx, ny, nz, dx, dy, dz, i)
+        pad = _pad_kernel(Nrow, nx, ny)
+        del Nrow
         if dft == "naive":
             Nhat = np.einsum("kq,jcqp,np->jckn", Wy, pad, Wx, optimize=True)
         else:

@@ -188,3 +188,89 @@ def test_argument_errors(hb):
         hb.demag(p, x.data_ptr(), None, y.data_ptr(), 0)
     assert e.value.status == hb.ESTATE
     hb.destroy(p)
+
+
+# ---------------------------------------------------------------------------------------------
+# Full-size configs of BASELINE.json, in the launch configuration bench.py times: sampled cells
+# against the direct real-space sum (T0, Eq.18), which the oracle computes one cell
+# at a time, plus the closed-form volume average for uniform magnetisation (pin P8) that holds
+# at any size.
+# ---------------------------------------------------------------------------------------------
+def _sampled_direct_check(hb, w, layers, ncells, states=(0,), tol=None):
+    import torch
+    tol = TOL[w.precision] if tol is None else tol
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B)
+    plan.build_tensor()
+    dt = torch.float32 if w.precision == "f32" else torch.float64
+    m_dev = torch.empty((w.B, 3, w.nz, w.ny, w.nx), dtype=dt, device="cuda")
+    m_np = {}
+    for b in range(w.B):
+        mb = w.m_rounded([b])[0]
+        m_dev[b] = torch.from_numpy(mb).to(dt).cuda()
+        if b in states:
+            m_np[b] = mb
+    h = plan.demag(m_dev, w.Ms)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(h).all())
+    rng = np.random.default_rng(w.seed)
+    worst = 0.0
+    for i in layers:
+        Nrow = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, i)
+        # corners, edges and random interior cells
+        cells = np.concatenate([[0, w.nx - 1, (w.ny - 1) * w.nx, w.ny * w.nx - 1, (w.ny // 2) * w.nx + w.nx // 2],
+                                rng.choice(w.nx * w.ny, size=ncells - 5, replace=False)]).astype(np.int32)
+        for b in states:
+            H0 = O.direct_cells(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m_np[b], w.Ms, i, cells, Nrow=Nrow)
+            Hb = h[b].double().cpu().numpy()
+            got = Hb[:, i].reshape(3, -1)[:, cells].T
+            # max|H_ref| over the whole field is not computable by the direct sum; the field of
+            # the GPU path itself bounds it to within the tolerance being tested
+            scale = np.abs(Hb).max()
+            worst = max(worst, float(np.abs(got - H0).max() / scale))
+        del Nrow
+    plan.close()
+    assert worst <= tol, worst
+    return worst
+
+
+def _uniform_average_check(hb, w, tol):
+    """<H>_volume = -Ms N_box m for uniform m (additivity of Eq.3); N_box from the oracle's
+    binary128 self-term of the bounding box."""
+    import torch
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=1)
+    plan.build_tensor()
+    dt = torch.float32 if w.precision == "f32" else torch.float64
+    box = np.array([w.nx * w.dx, w.ny * w.dy, w.dz.sum()])
+    hi, lo = O.tensor_point([0, 0, 0], box, box)
+    Ms = 8e5
+    for a in range(3):
+        m = torch.zeros((1, 3, w.nz, w.ny, w.nx), dtype=dt, device="cuda")
+        m[0, a] = 1.0
+        H = plan.demag(m, Ms).double()
+        dzt = torch.from_numpy(w.dz).cuda()
+        avg = (H[0] * dzt[None, :, None, None]).sum(dim=(1, 2, 3)).cpu().numpy() / (w.nx * w.ny * w.dz.sum())
+        want = np.zeros(3)
+        want[a] = -Ms * (hi[a] + lo[a])
+        assert np.abs(avg - want).max() <= tol * Ms, (a, avg, want)
+    plan.close()
+
+
+def test_config3_256x256x16_fp32_sampled(hb):
+    w = W.config(3)
+    _sampled_direct_check(hb, w, layers=[0, 9], ncells=40)
+    _uniform_average_check(hb, w, 2e-6)
+
+
+def test_config4_256x256x64_fp32_sampled(hb):
+    w = W.config(4)
+    _sampled_direct_check(hb, w, layers=[37], ncells=32)
+    _uniform_average_check(hb, w, 2e-6)
+
+
+def test_config4_equal_thickness_variant_uniform_average(hb):
+    _uniform_average_check(hb, W.config(4, "equal"), 2e-6)
+
+
+def test_config5_512x512x8_batch32_fp32_sampled(hb):
+    w = W.config(5)
+    _sampled_direct_check(hb, w, layers=[3], ncells=24, states=(0, 31))
