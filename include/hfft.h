@@ -148,7 +148,7 @@ hfft_status hfft_profile_read(hfft_plan *plan, double stage_ms[HFFT_NUM_STAGES],
 /*
  * Introspection for tests: copy one spectral bank plane N^_{ij}^{c}(k) to a
  * HOST array of n_k doubles, c in xx,yy,zz,xy,xz,yz = 0..5.  Element k =
- * ky * nx + kx for kx < nx, and 2ny * nx + ky for the Nyquist column kx = nx.
+ * kx * 2ny + ky, kx = 0..nx (Hermitian half spectrum along x), ky = 0..2ny-1.
  * The value is the real part for c < 4 and the imaginary part for c = 4, 5.
  * Synchronises the device.  Errors: EINVAL, ESTATE.
  */

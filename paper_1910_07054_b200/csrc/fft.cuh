@@ -1,15 +1,20 @@
-// fft.cuh -- shared-memory radix-4 (+ one radix-2) FFT building blocks.
+// fft.cuh -- register-resident Stockham FFT of one contiguous row, radix 8 (+ one radix 4 / 2 stage).
 //
-// Forward transforms are decimation-in-frequency: natural order in, digit-reversed order out,
-// in place in shared memory.  Inverse transforms are decimation-in-time on digit-reversed
-// input: natural order out.  Neither needs a reordering pass because the global-memory
-// load / store of each kernel applies the digit permutation row by row.
+// A row of N = 2^LOG2N complex numbers is transformed by TPR = N / R threads (R = 8, or N when
+// N < 8).  Thread j holds x[j + q TPR], q < R, in registers, does the radix-R butterflies of a
+// stage in registers, and exchanges data with the other threads of its row through shared
+// memory between stages (autosort: natural order in, natural order out, no digit reversal).
+// After the last stage thread j again holds X[j + q TPR].
 //
-// Zero padding (the circular convolution of Eq.20-24 is made linear by
-// padding nx -> 2nx, ny -> 2ny; reading A10) is implicit: the first radix-4 stage of a forward
-// transform reads only the two non-zero quarters of its input straight from global memory.
-// Cropping is fused the same way: the last radix-4 stage of an inverse transform computes only
-// the first half of its outputs and writes them straight to global memory.
+// Stage s has radix r_s and N_s = r_0 ... r_{s-1}.  Butterfly b (0 <= b < N / r_s) reads the
+// elements b + t N / r_s, t < r_s, multiplies them by exp(-+ 2 pi i t (b mod N_s) / (N_s r_s)),
+// takes the r_s-point DFT and writes output t to (b div N_s) N_s r_s + (b mod N_s) + t N_s.
+//
+// Zero padding (the circular convolution of Eq.20-24 is made linear by padding
+// nx -> 2nx, ny -> 2ny; reading A10) is implicit: with ZP the caller loads only q < R / 2 and the
+// first butterfly is specialised for a zero upper half -- no zero is ever loaded or stored.
+// Cropping is fused the same way: the caller of an inverse transform stores only q < R / 2, and
+// the arithmetic of the unused outputs is dead code the compiler removes.
 //
 // Sign convention (reading A11): forward e^{-2 pi i k n / N} unnormalised, inverse e^{+...}
 // unnormalised; the 1/(4 nx ny) lives in the tensor bank.
@@ -39,89 +44,131 @@ template <typename C> __device__ __forceinline__ C cmulc(C a, C b) {
 template <typename C> __device__ __forceinline__ C mul_mi(C a) { C r; r.x = a.y; r.y = -a.x; return r; }   // -i a
 template <typename C> __device__ __forceinline__ C mul_pi(C a) { C r; r.x = -a.y; r.y = a.x; return r; }   // +i a
 template <typename C> __device__ __forceinline__ C cconj(C a) { C r; r.x = a.x; r.y = -a.y; return r; }
+// multiplication by the stage's quarter turn: -i forward, +i inverse
+template <bool INV, typename C> __device__ __forceinline__ C mul_qt(C a) { return INV ? mul_pi(a) : mul_mi(a); }
+// a * w forward, a * conj(w) inverse (the tables hold exp(-2 pi i t / NT))
+template <bool INV, typename C> __device__ __forceinline__ C tmul(C a, C w) { return INV ? cmulc(a, w) : cmul(a, w); }
 
-// ---- digit permutation of the radix-(4,...,4[,2]) DIF --------------------------------------
-// reverse the order of S two-bit groups
-__device__ __forceinline__ unsigned rev_groups(unsigned q, int S) {
-    if (S == 0) return 0u;
-    unsigned r = __brev(q) >> (32 - 2 * S);
-    return ((r & 0x55555555u) << 1) | ((r >> 1) & 0x55555555u);
-}
-// frequency held at position p after the forward DIF
-template <int LOG2N> __device__ __forceinline__ int pos2freq(int p) {
-    constexpr int S = LOG2N / 2;
-    if (LOG2N & 1) return (int)(((unsigned)(p & 1) << (2 * S)) | rev_groups((unsigned)p >> 1, S));
-    return (int)rev_groups((unsigned)p, S);
-}
-// position at which frequency k sits
-template <int LOG2N> __device__ __forceinline__ int freq2pos(int k) {
-    constexpr int S = LOG2N / 2;
-    if (LOG2N & 1) return (int)((rev_groups((unsigned)k & ((1u << (2 * S)) - 1u), S) << 1) | ((unsigned)k >> (2 * S)));
-    return (int)rev_groups((unsigned)k, S);
-}
+// Shared-memory index swizzle.  Rows are accessed (a) at consecutive indices, (b) at stride 8
+// (stores after the first radix-8 stage) and (c) in runs of 8 at stride 64 (stores after the
+// second); XOR-ing bits 4..6 into bits 0..3 makes all three conflict free for 8-byte elements.
+// A bijection on [0, N) for every power of two N.
+__device__ __forceinline__ int swz(int i) { return i ^ ((i >> 4) & 7) ^ ((i >> 3) & 8); }
 
-// ---- radix-4 butterflies -------------------------------------------------------------------
-// forward DIF: y_m = (sum_r a_r (-i)^{rm}) * W^{jm}; caller applies the twiddles
-template <typename C> __device__ __forceinline__ void bfly4_fwd(C& a0, C& a1, C& a2, C& a3) {
-    C t0 = cadd(a0, a2), t1 = csub(a0, a2), t2 = cadd(a1, a3), t3 = csub(a1, a3);
+// ---- small DFTs in registers; ZH: the upper half of the inputs is zero (not read) ----------
+template <bool INV, bool ZH, typename C> __device__ __forceinline__ void dft2(C& a0, C& a1) {
+    if (ZH) { a1 = a0; return; }
+    C t = a0;
+    a0 = cadd(t, a1);
+    a1 = csub(t, a1);
+}
+template <bool INV, bool ZH, typename C> __device__ __forceinline__ void dft4(C& a0, C& a1, C& a2, C& a3) {
+    C t0, t1, t2, t3;
+    if (ZH) { t0 = a0; t1 = a0; t2 = a1; t3 = a1; }
+    else { t0 = cadd(a0, a2); t1 = csub(a0, a2); t2 = cadd(a1, a3); t3 = csub(a1, a3); }
+    C q = mul_qt<INV>(t3);
     a0 = cadd(t0, t2);
     a2 = csub(t0, t2);
-    C mt3 = mul_mi(t3);
-    a1 = cadd(t1, mt3);
-    a3 = csub(t1, mt3);
+    a1 = cadd(t1, q);
+    a3 = csub(t1, q);
 }
-// inverse DIT: y_r = sum_m b_m (+i)^{rm}
-template <typename C> __device__ __forceinline__ void bfly4_inv(C& b0, C& b1, C& b2, C& b3) {
-    C t0 = cadd(b0, b2), t1 = csub(b0, b2), t2 = cadd(b1, b3), t3 = csub(b1, b3);
-    b0 = cadd(t0, t2);
-    b2 = csub(t0, t2);
-    C pt3 = mul_pi(t3);
-    b1 = cadd(t1, pt3);
-    b3 = csub(t1, pt3);
+// X[2m] = DFT4(a_n + a_{n+4})[m], X[2m+1] = DFT4((a_n - a_{n+4}) W_8^n)[m]
+template <bool INV, bool ZH, typename T, typename C>
+__device__ __forceinline__ void dft8(C& a0, C& a1, C& a2, C& a3, C& a4, C& a5, C& a6, C& a7) {
+    const T h = (T)0.70710678118654752440;
+    C e0, e1, e2, e3, o0, o1, o2, o3;
+    if (ZH) { e0 = a0; e1 = a1; e2 = a2; e3 = a3; o0 = a0; o1 = a1; o2 = a2; o3 = a3; }
+    else {
+        e0 = cadd(a0, a4); e1 = cadd(a1, a5); e2 = cadd(a2, a6); e3 = cadd(a3, a7);
+        o0 = csub(a0, a4); o1 = csub(a1, a5); o2 = csub(a2, a6); o3 = csub(a3, a7);
+    }
+    // o1 *= W8, o2 *= W8^2, o3 *= W8^3 with W8 = exp(-+ i pi / 4)
+    if (!INV) {
+        o1 = mk<T>((o1.x + o1.y) * h, (o1.y - o1.x) * h);
+        o2 = mul_mi(o2);
+        o3 = mk<T>((o3.y - o3.x) * h, -(o3.x + o3.y) * h);
+    } else {
+        o1 = mk<T>((o1.x - o1.y) * h, (o1.x + o1.y) * h);
+        o2 = mul_pi(o2);
+        o3 = mk<T>(-(o3.x + o3.y) * h, (o3.x - o3.y) * h);
+    }
+    dft4<INV, false>(e0, e1, e2, e3);
+    dft4<INV, false>(o0, o1, o2, o3);
+    a0 = e0; a1 = o0; a2 = e1; a3 = o1; a4 = e2; a5 = o2; a6 = e3; a7 = o3;
 }
 
-// Twiddle table: tw[t] = exp(-2 pi i t / NT), t in [0, NT).  A transform of length N <= NT that
-// divides NT uses stride NT / N.
-template <typename C> __device__ __forceinline__ C ldtw(const C* __restrict__ tw, int idx) { return __ldg(tw + idx); }
+// ---- the row transform ------------------------------------------------------------------------
+template <typename T, int LOG2N, bool INV, bool ZP>
+struct RowFFT {
+    typedef HFFT_C C;
+    static constexpr int N = 1 << LOG2N;
+    static constexpr int LOG2R = LOG2N < 3 ? LOG2N : 3;
+    static constexpr int R = 1 << LOG2R;           // elements per thread
+    static constexpr int TPR = N / R;              // threads per row
+    static constexpr int LOG2TPR = LOG2N - LOG2R;
 
-// One in-place forward DIF radix-4 stage on block length L (Q = L / 4) for butterfly t of one
-// sequence whose element e lives at s[e * ES]; twiddle W_L^{jm} = tw[j m twmul].
-template <typename C>
-__device__ __forceinline__ void dif4_stage(C* s, const int ES, int t, int log2Q, const C* __restrict__ tw, int twmul) {
-    const int Q = 1 << log2Q;
-    const int j = t & (Q - 1);
-    const int base = ((t >> log2Q) << (log2Q + 2)) + j;
-    C a0 = s[(base) * ES], a1 = s[(base + Q) * ES], a2 = s[(base + 2 * Q) * ES], a3 = s[(base + 3 * Q) * ES];
-    bfly4_fwd(a0, a1, a2, a3);
-    if (log2Q > 0) {     // Q == 1: j == 0, twiddles are 1
-        const int w = j * twmul;
-        a1 = cmul(a1, ldtw(tw, w));
-        a2 = cmul(a2, ldtw(tw, 2 * w));
-        a3 = cmul(a3, ldtw(tw, 3 * w));
+    // twiddles of one butterfly: w[t] = tw[t k step], t = 1 .. RAD-1 (k step < NT / RAD)
+    template <int RAD>
+    static __device__ __forceinline__ void twiddles(C (&w)[8], const C* __restrict__ tw, int idx) {
+        w[1] = __ldg(tw + idx);
+        if (RAD >= 4) { w[2] = __ldg(tw + 2 * idx); w[3] = __ldg(tw + 3 * idx); }
+        if (RAD >= 8) {
+            w[4] = __ldg(tw + 4 * idx); w[5] = __ldg(tw + 5 * idx);
+            w[6] = __ldg(tw + 6 * idx); w[7] = __ldg(tw + 7 * idx);
+        }
     }
-    s[(base) * ES] = a0; s[(base + Q) * ES] = a1; s[(base + 2 * Q) * ES] = a2; s[(base + 3 * Q) * ES] = a3;
-}
-// One in-place inverse DIT radix-4 stage (conjugate twiddles first, then butterfly).
-template <typename C>
-__device__ __forceinline__ void dit4_stage(C* s, const int ES, int t, int log2Q, const C* __restrict__ tw, int twmul) {
-    const int Q = 1 << log2Q;
-    const int j = t & (Q - 1);
-    const int base = ((t >> log2Q) << (log2Q + 2)) + j;
-    C b0 = s[(base) * ES], b1 = s[(base + Q) * ES], b2 = s[(base + 2 * Q) * ES], b3 = s[(base + 3 * Q) * ES];
-    if (log2Q > 0) {
-        const int w = j * twmul;
-        b1 = cmulc(b1, ldtw(tw, w));
-        b2 = cmulc(b2, ldtw(tw, 2 * w));
-        b3 = cmulc(b3, ldtw(tw, 3 * w));
+
+    // One stage of radix 2^LR at N_s = 2^LNS, followed (unless it is the last) by the exchange.
+    template <int LNS, int LR>
+    static __device__ __forceinline__ void stage(C (&v)[R], C* __restrict__ srow, int j, const C* __restrict__ tw,
+                                                 int twmul) {
+        constexpr int RAD = 1 << LR;
+        constexpr int U = R / RAD;                  // butterflies per thread
+        constexpr int NS = 1 << LNS;
+        constexpr bool FIRST = LNS == 0;
+        constexpr bool LAST = LNS + LR == LOG2N;
+        int pos[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const int b = j + u * TPR;
+            const int k = b & (NS - 1);
+            if constexpr (!FIRST) {
+                C w[8];
+                twiddles<RAD>(w, tw, k * ((N >> (LNS + LR)) * twmul));
+#pragma unroll
+                for (int t = 1; t < RAD; ++t) v[u + t * U] = tmul<INV>(v[u + t * U], w[t]);
+            }
+            if constexpr (RAD == 8)
+                dft8<INV, ZP && FIRST, T>(v[u], v[u + U], v[u + 2 * U], v[u + 3 * U], v[u + 4 * U], v[u + 5 * U],
+                                          v[u + 6 * U], v[u + 7 * U]);
+            else if constexpr (RAD == 4)
+                dft4<INV, ZP && FIRST>(v[u], v[u + U], v[u + 2 * U], v[u + 3 * U]);
+            else
+                dft2<INV, ZP && FIRST>(v[u], v[u + U]);
+            pos[u] = ((b >> LNS) << (LNS + LR)) + k;
+        }
+        if constexpr (!LAST) {
+            __syncthreads();                        // earlier readers of the row are done
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+#pragma unroll
+                for (int t = 0; t < RAD; ++t) srow[swz(pos[u] + t * NS)] = v[u + t * U];
+            __syncthreads();
+#pragma unroll
+            for (int q = 0; q < R; ++q) v[q] = srow[swz(j + q * TPR)];
+            constexpr int LEFT = LOG2N - LNS - LR;  // > 0 here
+            constexpr int NLR = LEFT >= 3 ? 3 : LEFT;
+            stage<LNS + LR, NLR>(v, srow, j, tw, twmul);
+        }
+        // LAST: output t of butterfly u is X[j + (u + t U) TPR] and already sits in v[u + t U]
     }
-    bfly4_inv(b0, b1, b2, b3);
-    s[(base) * ES] = b0; s[(base + Q) * ES] = b1; s[(base + 2 * Q) * ES] = b2; s[(base + 3 * Q) * ES] = b3;
-}
-// radix-2 stage on blocks of length 2 (no twiddles): butterfly t touches elements 2t, 2t+1
-template <typename C> __device__ __forceinline__ void r2_stage(C* s, const int ES, int t) {
-    C a0 = s[(2 * t) * ES], a1 = s[(2 * t + 1) * ES];
-    s[(2 * t) * ES] = cadd(a0, a1);
-    s[(2 * t + 1) * ES] = csub(a0, a1);
-}
+
+    // v[q] = x[j + q TPR] (q < R / 2 if ZP) on entry, X[j + q TPR] on return.  Every thread of the
+    // CTA must call this together (it contains __syncthreads); srow is this row's N-element buffer.
+    static __device__ __forceinline__ void run(C (&v)[R], C* __restrict__ srow, int j, const C* __restrict__ tw,
+                                               int twmul) {
+        stage<0, LOG2R>(v, srow, j, tw, twmul);
+    }
+};
 
 }  // namespace hfft

@@ -243,9 +243,7 @@ template <typename T>
 static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, void* h, cudaStream_t st) {
     unsigned char* ws = static_cast<unsigned char*>(p->ws);
     const int planes = 3 * p->nz * p->batch;
-    const int nrows = planes * p->ny;
-    void* xmain = ws + p->ws_xhat;
-    void* xnyq = ws + p->ws_xhat + (size_t)nrows * p->nx * 2 * sizeof(T);
+    void* xhat = ws + p->ws_xhat;
     void* spec = ws + p->ws_spec;
     cudaEvent_t* ev = nullptr;
     if (p->profiling) {
@@ -256,11 +254,11 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
 #define STAGE(idx, call)                                                            \
     if (ev && (e = cudaEventRecord(ev[idx], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e); \
     if ((e = (call)) != cudaSuccess) return fail_cuda(p, #call, e);
-    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xmain, xnyq, p->log2nx, nrows, p->ny, p->nz, Ms, p->tw_x, st)))
-    STAGE(1, (launch_ffty_fwd<T, true>(xmain, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
+    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, st)))
+    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
     STAGE(2, (launch_coupling<T>(p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded, p->num_sms, st)))
-    STAGE(3, (launch_iffty<T>(spec, xmain, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
-    STAGE(4, (launch_ifftx<T>(xmain, xnyq, (T*)h, p->log2nx, nrows, p->tw_x, st)))
+    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
+    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, st)))
 #undef STAGE
     if (ev) {
         if ((e = cudaEventRecord(ev[HFFT_NUM_STAGES], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);

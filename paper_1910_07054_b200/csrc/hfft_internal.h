@@ -14,20 +14,20 @@ namespace hfft {
 template <typename T> struct MsParam { T v[HFFT_MAX_NZ]; };
 
 // ---- fft_kernels.cu ----
-// forward x: `in` real rows (nx reals if ZP, 2nx if not) -> main [nrows][nx] + Nyquist [nrows]
+// forward x: `in` real rows [nplanes][rows_per_plane][nx if ZP else 2nx] -> X^ [nplanes][nx+1][rows_per_plane]
 template <typename T, bool ZP>
-cudaError_t launch_fftx_fwd(const T* in, void* out_main, void* out_nyq, int log2nx, int nrows, int rows_per_plane,
-                            int nz, const double* ms_host, const void* tw2nx, cudaStream_t st);
+cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, int rows_per_plane, int nz,
+                            const double* ms_host, const void* tw2nx, cudaStream_t st);
 template <typename T>
-cudaError_t launch_ifftx(const void* in_main, const void* in_nyq, T* out, int log2nx, int nrows, const void* tw2nx,
+cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw2nx,
                          cudaStream_t st);
-// forward y: row side (main [nplanes*rows][nx] + Nyquist [nplanes*rows]) -> k side [nplanes][ks];
+// forward y: X^ rows [nplanes * (nx+1)][N/2 if ZP else N] -> k side [nplanes][ks], k = kx * N + ky;
 // nz_rot > 0 multiplies the z-component planes by i
 template <typename T, bool ZP>
-cudaError_t launch_ffty_fwd(const void* in, void* out, int nx, int log2N, int nplanes, int nz_rot, long long ks,
+cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int nplanes, int nz_rot, long long ks,
                             const void* twN, cudaStream_t st);
 template <typename T>
-cudaError_t launch_iffty(const void* in, void* out, int nx, int log2N, int nplanes, int nz_rot, long long ks,
+cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
                          const void* twN, cudaStream_t st);
 
 // ---- coupling.cu ----

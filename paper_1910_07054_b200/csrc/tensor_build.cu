@@ -216,8 +216,7 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
             assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
                                                   make_double2(coef.hi, coef.lo));
             HFFT_CK(cudaGetLastError());
-            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, d_X + (size_t)jn * 6 * 2 * ny * nx, g.log2nx,
-                                                    jn * 6 * 2 * ny, 2 * ny, 0, nullptr, tw2nx, st)));
+            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, g.log2nx, jn * 6, 2 * ny, 0, nullptr, tw2nx, st)));
             HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, tw2ny, st)));
             dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
             if (g.prec == HFFT_F32)

@@ -60,9 +60,8 @@ def _oracle_nhat(w, i):
     q = np.arange(-(ny - 1), ny)
     pad[:, :, (q % (2 * ny))[:, None], (p % (2 * nx))[None, :]] = row
     Nh = np.fft.fft2(pad, axes=(-2, -1))
-    main = Nh[..., :, :nx].reshape(w.nz, 6, -1)
-    nyq = Nh[..., :, nx]
-    return np.concatenate([main, nyq], axis=-1)
+    # library order: k = kx * 2ny + ky, kx = 0..nx
+    return np.swapaxes(Nh[..., :, :nx + 1], -1, -2).reshape(w.nz, 6, -1)
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
