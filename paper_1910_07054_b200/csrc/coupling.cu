@@ -81,9 +81,9 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
         __syncthreads();
 
         for (int i = warp; i < nz; i += nwarps) {
-            T hx[KPT][2], hy[KPT][2], hz[KPT][2];
+            C hx[KPT], hy[KPT], hz[KPT];
 #pragma unroll
-            for (int e = 0; e < KPT; ++e) { hx[e][0] = hx[e][1] = hy[e][0] = hy[e][1] = hz[e][0] = hz[e][1] = (T)0; }
+            for (int e = 0; e < KPT; ++e) hx[e] = hy[e] = hz[e] = mk<T>((T)0, (T)0);
             const T* bt = bank + ((tile * nz + i) * nz) * (6LL * TK) + lane * KPT;
 #pragma unroll 2
             for (int j = 0; j < nz; ++j) {
@@ -114,35 +114,150 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                 }
 #pragma unroll
                 for (int e = 0; e < KPT; ++e) {
-                    hx[e][0] += a[0][e] * m[0][e].x + a[3][e] * m[1][e].x + a[4][e] * m[2][e].x;
-                    hx[e][1] += a[0][e] * m[0][e].y + a[3][e] * m[1][e].y + a[4][e] * m[2][e].y;
-                    hy[e][0] += a[3][e] * m[0][e].x + a[1][e] * m[1][e].x + a[5][e] * m[2][e].x;
-                    hy[e][1] += a[3][e] * m[0][e].y + a[1][e] * m[1][e].y + a[5][e] * m[2][e].y;
-                    hz[e][0] += a[2][e] * m[2][e].x - a[4][e] * m[0][e].x - a[5][e] * m[1][e].x;
-                    hz[e][1] += a[2][e] * m[2][e].y - a[4][e] * m[0][e].y - a[5][e] * m[1][e].y;
+                    hx[e] = caxpy_s(a[0][e], m[0][e], hx[e]); hx[e] = caxpy_s(a[3][e], m[1][e], hx[e]); hx[e] = caxpy_s(a[4][e], m[2][e], hx[e]);
+                    hy[e] = caxpy_s(a[3][e], m[0][e], hy[e]); hy[e] = caxpy_s(a[1][e], m[1][e], hy[e]); hy[e] = caxpy_s(a[5][e], m[2][e], hy[e]);
+                    hz[e] = caxpy_s(a[2][e], m[2][e], hz[e]); hz[e] = caxpy_s(-a[4][e], m[0][e], hz[e]); hz[e] = caxpy_s(-a[5][e], m[1][e], hz[e]);
                 }
             }
             C* ox = sp + (long long)(0 * nz + i) * ks + lane * KPT;
             C* oy = sp + (long long)(1 * nz + i) * ks + lane * KPT;
             C* oz = sp + (long long)(2 * nz + i) * ks + lane * KPT;
             if (SWZ && sizeof(T) == 4) {
-                reinterpret_cast<float4*>(ox)[0] = make_float4(hx[0][0], hx[0][1], hx[1 % KPT][0], hx[1 % KPT][1]);
-                reinterpret_cast<float4*>(ox)[1] = make_float4(hx[2 % KPT][0], hx[2 % KPT][1], hx[3 % KPT][0], hx[3 % KPT][1]);
-                reinterpret_cast<float4*>(oy)[0] = make_float4(hy[0][0], hy[0][1], hy[1 % KPT][0], hy[1 % KPT][1]);
-                reinterpret_cast<float4*>(oy)[1] = make_float4(hy[2 % KPT][0], hy[2 % KPT][1], hy[3 % KPT][0], hy[3 % KPT][1]);
-                reinterpret_cast<float4*>(oz)[0] = make_float4(hz[0][0], hz[0][1], hz[1 % KPT][0], hz[1 % KPT][1]);
-                reinterpret_cast<float4*>(oz)[1] = make_float4(hz[2 % KPT][0], hz[2 % KPT][1], hz[3 % KPT][0], hz[3 % KPT][1]);
+                reinterpret_cast<float4*>(ox)[0] = make_float4(hx[0].x, hx[0].y, hx[1 % KPT].x, hx[1 % KPT].y);
+                reinterpret_cast<float4*>(ox)[1] = make_float4(hx[2 % KPT].x, hx[2 % KPT].y, hx[3 % KPT].x, hx[3 % KPT].y);
+                reinterpret_cast<float4*>(oy)[0] = make_float4(hy[0].x, hy[0].y, hy[1 % KPT].x, hy[1 % KPT].y);
+                reinterpret_cast<float4*>(oy)[1] = make_float4(hy[2 % KPT].x, hy[2 % KPT].y, hy[3 % KPT].x, hy[3 % KPT].y);
+                reinterpret_cast<float4*>(oz)[0] = make_float4(hz[0].x, hz[0].y, hz[1 % KPT].x, hz[1 % KPT].y);
+                reinterpret_cast<float4*>(oz)[1] = make_float4(hz[2 % KPT].x, hz[2 % KPT].y, hz[3 % KPT].x, hz[3 % KPT].y);
             } else {
 #pragma unroll
-                for (int e = 0; e < KPT; ++e) {
-                    ox[e] = mk<T>(hx[e][0], hx[e][1]);
-                    oy[e] = mk<T>(hy[e][0], hy[e][1]);
-                    oz[e] = mk<T>(hz[e][0], hz[e][1]);
-                }
+                for (int e = 0; e < KPT; ++e) { ox[e] = hx[e]; oy[e] = hy[e]; oz[e] = hz[e]; }
             }
         }
         __syncthreads();   // every warp is done with the tile in shared memory
     }
+}
+
+// ------------------------------------------------------------------------------------------
+// Batched mode (B magnetisation states per call, BASELINE config 5): per wavevector the coupling
+// is the real (3nz x 3nz) matrix times 2B real columns.  The bank of a k-tile is read from HBM
+// ONCE and kept in registers: a warp owns target layer i, a lane owns one wavevector and holds
+// the 6 nz reals a^c_ij(k) of its (i, k) for all source layers j.  The states stream through a
+// STAGES-deep cp.async ring of M^ tiles in shared memory ([3 nz][32] complex each); per state a
+// thread does 18 nz FMAs into 6 accumulators and writes H^ of its (i, k) in place.
+// Tile = 32 wavevectors (hfft_api.cu picks tile_k = 32 when this kernel applies).
+// ------------------------------------------------------------------------------------------
+template <int N> __device__ __forceinline__ void cp_async_wait_group() {
+    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
+
+template <typename T, int NZ, int STAGES>
+__global__ void __launch_bounds__(32 * NZ)
+coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int batch, long long n_tiles,
+                        long long ks) {
+    typedef HFFT_C C;
+    constexpr int TK = 32, NP = 3 * NZ;
+    constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk
+    constexpr int CPP = TK / CHUNK_C;                     // chunks per plane row
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* sm = reinterpret_cast<C*>(smem_raw);               // [STAGES][NP][TK]
+    const int tid = threadIdx.x, lane = tid & 31, i = tid >> 5;
+
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        C* sp = spec + tile * TK;
+        auto issue = [&](int b) {
+            if (b < batch) {
+                C* dst = sm + (b % STAGES) * (NP * TK);
+                const C* src = sp + (long long)b * NP * ks;
+                for (int w = tid; w < NP * CPP; w += 32 * NZ) {
+                    const int lp = w / CPP, ch = w - lp * CPP;
+                    cp_async16(dst + lp * TK + ch * CHUNK_C, src + (long long)lp * ks + ch * CHUNK_C);
+                }
+            }
+            cp_async_commit();
+        };
+#pragma unroll
+        for (int s = 0; s < STAGES - 1; ++s) issue(s);
+
+        T a[NZ][6];
+        const T* bt = bank + ((tile * NZ + i) * NZ) * (6LL * TK) + lane;
+#pragma unroll
+        for (int j = 0; j < NZ; ++j)
+#pragma unroll
+            for (int c = 0; c < 6; ++c) a[j][c] = __ldcs(bt + (j * 6 + c) * TK);
+
+        for (int b = 0; b < batch; ++b) {
+            issue(b + STAGES - 1);
+            cp_async_wait_group<STAGES - 1>();
+            __syncthreads();
+            const C* st = sm + (b % STAGES) * (NP * TK) + lane;
+            C hx = mk<T>((T)0, (T)0), hy = hx, hz = hx;
+#pragma unroll
+            for (int j = 0; j < NZ; ++j) {
+                const C mx = st[(0 * NZ + j) * TK], my = st[(1 * NZ + j) * TK], mz = st[(2 * NZ + j) * TK];
+                hx = caxpy(a[j][0], mx, hx); hx = caxpy(a[j][3], my, hx); hx = caxpy(a[j][4], mz, hx);
+                hy = caxpy(a[j][3], mx, hy); hy = caxpy(a[j][1], my, hy); hy = caxpy(a[j][5], mz, hy);
+                hz = caxpy(a[j][2], mz, hz); hz = caxpy(-a[j][4], mx, hz); hz = caxpy(-a[j][5], my, hz);
+            }
+            C* o = sp + (long long)b * NP * ks + lane;
+            o[(long long)(0 * NZ + i) * ks] = hx;
+            o[(long long)(1 * NZ + i) * ks] = hy;
+            o[(long long)(2 * NZ + i) * ks] = hz;
+            __syncthreads();   // every warp is done with this stage before it is refilled
+        }
+        cp_async_wait_group<0>();
+    }
+}
+
+// the batched kernel keeps 6 nz reals of the bank per thread: at most 96 32-bit registers
+bool coupling_batched_applies(int nz, int batch, size_t elem) {
+    return batch > 1 && (size_t)6 * nz * elem <= 96 * 4;
+}
+
+template <typename T, int NZ>
+static cudaError_t launch_coupling_batched_nz(const void* bank, void* spec, int batch, long long n_tiles,
+                                              long long ks, int num_sms, cudaStream_t st) {
+    typedef HFFT_C C;
+    constexpr int STAGES = 4;
+    auto kern = coupling_batched_kernel<T, NZ, STAGES>;
+    const size_t smem = (size_t)STAGES * 3 * NZ * 32 * sizeof(C);
+    static int occ_blocks = 0;
+    cudaError_t err;
+    if (occ_blocks == 0) {
+        if (smem > 48 * 1024) {
+            err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return err;
+        }
+        int nb = 0;
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 32 * NZ, smem);
+        if (err != cudaSuccess) return err;
+        occ_blocks = nb < 1 ? 1 : nb;
+    }
+    long long grid = (long long)num_sms * occ_blocks;
+    if (grid > n_tiles) grid = n_tiles;
+    kern<<<(unsigned)grid, 32 * NZ, smem, st>>>((const T*)bank, (C*)spec, batch, n_tiles, ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+static cudaError_t launch_coupling_batched(const void* bank, void* spec, int nz, int batch, long long n_tiles,
+                                           long long ks, int num_sms, cudaStream_t st) {
+#define HFFT_NZ_CASE(V) case V: return launch_coupling_batched_nz<T, V>(bank, spec, batch, n_tiles, ks, num_sms, st);
+    switch (nz) {
+        HFFT_NZ_CASE(1) HFFT_NZ_CASE(2) HFFT_NZ_CASE(3) HFFT_NZ_CASE(4) HFFT_NZ_CASE(5) HFFT_NZ_CASE(6)
+        HFFT_NZ_CASE(7) HFFT_NZ_CASE(8)
+        default: break;
+    }
+    if constexpr (sizeof(T) == 4) {
+        switch (nz) {
+            HFFT_NZ_CASE(9) HFFT_NZ_CASE(10) HFFT_NZ_CASE(11) HFFT_NZ_CASE(12) HFFT_NZ_CASE(13) HFFT_NZ_CASE(14)
+            HFFT_NZ_CASE(15) HFFT_NZ_CASE(16)
+            default: break;
+        }
+    }
+#undef HFFT_NZ_CASE
+    return cudaErrorInvalidValue;
 }
 
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem) { return (size_t)3 * nz * tile_k * 2 * elem; }
@@ -181,6 +296,8 @@ template <typename T>
 cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
                             long long ks, int num_sms, cudaStream_t st) {
     constexpr int KV = 16 / sizeof(T);
+    if (tile_k == 32 && coupling_batched_applies(nz, batch, sizeof(T)))
+        return launch_coupling_batched<T>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
     if (tile_k == 32 * KV) return launch_coupling_k<T, KV>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
     if (tile_k == 32) return launch_coupling_k<T, 1>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
     return cudaErrorInvalidValue;

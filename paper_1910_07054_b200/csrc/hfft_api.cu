@@ -100,6 +100,7 @@ static void plan_sizes(hfft_plan* p) {
     p->tile_k = (p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148)) ? wide : 32;
     while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
     if (p->tile_k != wide) p->tile_k = 32;
+    if (coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
     p->n_tiles = (p->n_k + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
     p->bank_bytes = (size_t)6 * p->nz * p->nz * (size_t)p->n_k_padded * e;

@@ -36,6 +36,8 @@ template <typename T>
 cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
                             long long ks, int num_sms, cudaStream_t st);
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem);
+// batched register-resident-bank kernel (B > 1, small nz); it needs tile_k == 32
+bool coupling_batched_applies(int nz, int batch, size_t elem);
 
 // ---- tensor_build.cu ----
 struct BuildGeom {

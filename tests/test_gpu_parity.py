@@ -117,6 +117,9 @@ SHAPES = [
     # nx, ny, nz, B   -- ragged (nx != ny), tiny, single layer, odd layer counts, several tiles + tail
     (2, 2, 1, 1), (2, 4, 2, 1), (4, 2, 3, 2), (8, 32, 5, 1), (32, 8, 1, 3), (16, 16, 7, 2), (64, 32, 4, 1),
     (128, 16, 2, 1), (32, 128, 3, 1),
+    # batched register-resident-bank coupling (B > 1): nz = 8 (config 5's), the fp32 / fp64 limits 16 / 8,
+    # and an nz beyond the fp64 limit (falls back to the per-state kernel)
+    (16, 16, 8, 5), (8, 16, 16, 3), (8, 8, 12, 2), (64, 64, 8, 7),
 ]
 
 
