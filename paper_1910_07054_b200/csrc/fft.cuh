@@ -103,8 +103,27 @@ template <bool INV, typename C> __device__ __forceinline__ C tmul(C a, C w) { re
 // Shared-memory index swizzle.  Rows are accessed (a) at consecutive indices, (b) at stride 8
 // (stores after the first radix-8 stage) and (c) in runs of 8 at stride 64 (stores after the
 // second); XOR-ing bits 4..6 into bits 0..3 makes all three conflict free for 8-byte elements.
-// A bijection on [0, N) for every power of two N.
-__device__ __forceinline__ int swz(int i) { return i ^ ((i >> 4) & 7) ^ ((i >> 3) & 8); }
+// A bijection on [0, N) for every power of two N, and LINEAR over GF(2): swz(a ^ b) = swz(a) ^
+// swz(b).  Every index used below is a sum of a per-thread part and a compile-time part that
+// occupy disjoint bits, so an address is (per-thread base) XOR (compile-time constant): one
+// LOP3 per shared-memory access, with the base computed once per kernel.
+__host__ __device__ constexpr int swz(int i) { return i ^ ((i >> 4) & 7) ^ ((i >> 3) & 8); }
+
+// shared-memory access by 32-bit shared-space address (the XOR arithmetic is done on integers)
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+template <typename C> __device__ __forceinline__ C lds(unsigned addr);
+template <> __device__ __forceinline__ float2 lds<float2>(unsigned addr) {
+    float2 v; asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(addr) : "memory"); return v;
+}
+template <> __device__ __forceinline__ double2 lds<double2>(unsigned addr) {
+    double2 v; asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr) : "memory"); return v;
+}
+__device__ __forceinline__ void sts(unsigned addr, float2 v) {
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(addr), "f"(v.x), "f"(v.y) : "memory");
+}
+__device__ __forceinline__ void sts(unsigned addr, double2 v) {
+    asm volatile("st.shared.v2.f64 [%0], {%1, %2};" ::"r"(addr), "d"(v.x), "d"(v.y) : "memory");
+}
 
 // ---- small DFTs in registers; ZH: the upper half of the inputs is zero (not read) ----------
 template <bool INV, bool ZH, typename C> __device__ __forceinline__ void dft2(C& a0, C& a1) {
@@ -149,8 +168,19 @@ __device__ __forceinline__ void dft8(C& a0, C& a1, C& a2, C& a3, C& a4, C& a5, C
     a0 = e0; a1 = o0; a2 = e1; a3 = o1; a4 = e2; a5 = o2; a6 = e3; a7 = o3;
 }
 
+
 // ---- the row transform ------------------------------------------------------------------------
-template <typename T, int LOG2N, bool INV, bool ZP>
+// Everything that depends only on the thread (not on the row) lives in a Ctx that a persistent
+// kernel sets up once: the twiddles of the thread's butterflies (registers if REGTW, else read
+// from the thread's column of a per-thread table with immediate offsets) and the swizzled
+// shared-memory base addresses.  Per row a thread then executes the butterflies, one LOP3 per
+// shared-memory access and ONE barrier per exchange (two buffers per row, used alternately).
+//
+// Per-thread twiddle table (host: thread_twiddle_table in hfft_api.cu): for the stages after the
+// first, in order, slot = OFF(stage) + u (RAD - 1) + (t - 1) holds, for thread j < TPR,
+//     exp(-2 pi i t k / (N_s RAD)),  k = (j + u TPR) mod N_s,
+// stored [slot][j] so that the TPR threads of a row read consecutive elements.
+template <typename T, int LOG2N, bool INV, bool ZP, bool REGTW>
 struct RowFFT {
     typedef HFFT_C C;
     static constexpr int N = 1 << LOG2N;
@@ -158,37 +188,86 @@ struct RowFFT {
     static constexpr int R = 1 << LOG2R;           // elements per thread
     static constexpr int TPR = N / R;              // threads per row
     static constexpr int LOG2TPR = LOG2N - LOG2R;
+    static constexpr int SH = sizeof(C) == 8 ? 3 : 4;
+    static constexpr unsigned BUF_BYTES = (unsigned)N * sizeof(C);     // one exchange buffer of a row
+    static constexpr unsigned ROW_BYTES = 2 * BUF_BYTES;               // a row's two buffers; rows are aligned to this
 
-    // twiddles of one butterfly: w[t] = tw[t k step], t = 1 .. RAD-1 (k step < NT / RAD)
-    template <int RAD>
-    static __device__ __forceinline__ void twiddles(C (&w)[8], const C* __restrict__ tw, int idx) {
-        w[1] = __ldg(tw + idx);
-        if (RAD >= 4) { w[2] = __ldg(tw + 2 * idx); w[3] = __ldg(tw + 3 * idx); }
-        if (RAD >= 8) {
-            w[4] = __ldg(tw + 4 * idx); w[5] = __ldg(tw + 5 * idx);
-            w[6] = __ldg(tw + 6 * idx); w[7] = __ldg(tw + 7 * idx);
+    static __host__ __device__ constexpr int lr_at(int lns) { return lns == 0 ? LOG2R : (LOG2N - lns >= 3 ? 3 : LOG2N - lns); }
+    static __host__ __device__ constexpr int stages() { int n = 0; for (int l = 0; l < LOG2N; l += lr_at(l)) ++n; return n; }
+    // twiddle slots used by the stages that start below lns
+    static __host__ __device__ constexpr int slots_before(int lns) {
+        int n = 0;
+        for (int l = lr_at(0); l < lns; l += lr_at(l)) n += (R >> lr_at(l)) * ((1 << lr_at(l)) - 1);
+        return n;
+    }
+    static constexpr int NSTAGES = stages();
+    static constexpr int EXCH = NSTAGES - 1;                           // exchanges per row
+    static constexpr int NSLOTS = slots_before(LOG2N);
+
+    struct Ctx {
+        C tw[NSLOTS > 0 ? NSLOTS : 1];             // REGTW only
+        const C* twp;                              // twt + j
+        unsigned st[NSTAGES][R];                   // st[s][u]: store base of butterfly u after stage s
+        unsigned ld;                               // load base: element j of the row
+    };
+
+    // the row synchronises among its own threads only: one warp (or less) when TPR <= 32
+    static __device__ __forceinline__ void sync() {
+        if (TPR <= 32) __syncwarp(); else __syncthreads();
+    }
+
+    template <int LNS, int SIDX>
+    static __device__ __forceinline__ void init_stage(Ctx& c, unsigned rowaddr, int j, int rx) {
+        constexpr int LR = lr_at(LNS);
+        if constexpr (LNS + LR < LOG2N) {
+            constexpr int U = R >> LR, NS = 1 << LNS;
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int b = j + u * TPR;
+                const int pos = ((b >> LNS) << (LNS + LR)) + (b & (NS - 1));
+                c.st[SIDX][u] = rowaddr ^ ((unsigned)(swz(pos) ^ rx) << SH);
+            }
+            init_stage<LNS + LR, SIDX + 1>(c, rowaddr, j, rx);
         }
     }
 
-    // One stage of radix 2^LR at N_s = 2^LNS, followed (unless it is the last) by the exchange.
-    template <int LNS, int LR>
-    static __device__ __forceinline__ void stage(C (&v)[R], C* __restrict__ srow, int j, const C* __restrict__ tw,
-                                                 int twmul) {
+    // rowaddr: shared-space address of the row's buffer pair (ROW_BYTES aligned); rx < min(16, N)
+    // is XOR-ed into every element index of the row (lets a caller read the rows "transposed",
+    // lanes along rows, without bank conflicts); twt: per-thread twiddle table.
+    static __device__ __forceinline__ void init(Ctx& c, unsigned rowaddr, int j, int rx, const C* __restrict__ twt) {
+        c.ld = rowaddr ^ ((unsigned)(swz(j) ^ rx) << SH);
+        c.twp = twt + j;
+        if constexpr (REGTW) {
+#pragma unroll
+            for (int sl = 0; sl < NSLOTS; ++sl) c.tw[sl] = __ldg(twt + sl * TPR + j);
+        }
+        init_stage<0, 0>(c, rowaddr, j, rx);
+    }
+
+    // shared-space address of element (j + q TPR) of the row in buffer `par`
+    template <int PAR>
+    static __device__ __forceinline__ unsigned elem_addr(const Ctx& c, int q) {
+        return c.ld ^ (((unsigned)swz(q * TPR) << SH) ^ (PAR ? BUF_BYTES : 0u));
+    }
+
+    template <int LNS, int SIDX, int PAR>
+    static __device__ __forceinline__ void stage(C (&v)[R], const Ctx& c) {
+        constexpr int LR = lr_at(LNS);
         constexpr int RAD = 1 << LR;
         constexpr int U = R / RAD;                  // butterflies per thread
         constexpr int NS = 1 << LNS;
         constexpr bool FIRST = LNS == 0;
         constexpr bool LAST = LNS + LR == LOG2N;
-        int pos[U];
+        constexpr int OFF = slots_before(LNS);
 #pragma unroll
         for (int u = 0; u < U; ++u) {
-            const int b = j + u * TPR;
-            const int k = b & (NS - 1);
             if constexpr (!FIRST) {
-                C w[8];
-                twiddles<RAD>(w, tw, k * ((N >> (LNS + LR)) * twmul));
 #pragma unroll
-                for (int t = 1; t < RAD; ++t) v[u + t * U] = tmul<INV>(v[u + t * U], w[t]);
+                for (int t = 1; t < RAD; ++t) {
+                    const int sl = OFF + u * (RAD - 1) + (t - 1);
+                    const C w = REGTW ? c.tw[sl] : __ldg(c.twp + sl * TPR);
+                    v[u + t * U] = tmul<INV>(v[u + t * U], w);
+                }
             }
             if constexpr (RAD == 8)
                 dft8<INV, ZP && FIRST, T>(v[u], v[u + U], v[u + 2 * U], v[u + 3 * U], v[u + 4 * U], v[u + 5 * U],
@@ -197,29 +276,28 @@ struct RowFFT {
                 dft4<INV, ZP && FIRST>(v[u], v[u + U], v[u + 2 * U], v[u + 3 * U]);
             else
                 dft2<INV, ZP && FIRST>(v[u], v[u + U]);
-            pos[u] = ((b >> LNS) << (LNS + LR)) + k;
         }
         if constexpr (!LAST) {
-            __syncthreads();                        // earlier readers of the row are done
+            // output t of butterfly u goes to pos(u) + t N_s; pos has zero bits where t N_s lives
 #pragma unroll
             for (int u = 0; u < U; ++u)
 #pragma unroll
-                for (int t = 0; t < RAD; ++t) srow[swz(pos[u] + t * NS)] = v[u + t * U];
-            __syncthreads();
+                for (int t = 0; t < RAD; ++t)
+                    sts(c.st[SIDX][u] ^ (((unsigned)swz(t * NS) << SH) ^ (PAR ? BUF_BYTES : 0u)), v[u + t * U]);
+            sync();
 #pragma unroll
-            for (int q = 0; q < R; ++q) v[q] = srow[swz(j + q * TPR)];
-            constexpr int LEFT = LOG2N - LNS - LR;  // > 0 here
-            constexpr int NLR = LEFT >= 3 ? 3 : LEFT;
-            stage<LNS + LR, NLR>(v, srow, j, tw, twmul);
+            for (int q = 0; q < R; ++q) v[q] = lds<C>(elem_addr<PAR>(c, q));
+            stage<LNS + LR, SIDX + 1, PAR ^ 1>(v, c);
         }
         // LAST: output t of butterfly u is X[j + (u + t U) TPR] and already sits in v[u + t U]
     }
 
     // v[q] = x[j + q TPR] (q < R / 2 if ZP) on entry, X[j + q TPR] on return.  Every thread of the
-    // CTA must call this together (it contains __syncthreads); srow is this row's N-element buffer.
-    static __device__ __forceinline__ void run(C (&v)[R], C* __restrict__ srow, int j, const C* __restrict__ tw,
-                                               int twmul) {
-        stage<0, LOG2R>(v, srow, j, tw, twmul);
+    // row (of the CTA if TPR > 32) must call this together.  Exchange e uses buffer e & 1, so the
+    // only hazard between consecutive rows is an odd number of exchanges: one more barrier then.
+    static __device__ __forceinline__ void run(C (&v)[R], const Ctx& c) {
+        stage<0, 0, 0>(v, c);
+        if constexpr (EXCH & 1) sync();
     }
 };
 

@@ -14,195 +14,329 @@
 //   M^ (after S2)   [plane][KS] C, element k = kx * 2ny + ky
 // The z-component planes of M^ hold i*M_z (and H^ holds i*H_z) so that the layer coupling is a
 // real matrix acting on real and imaginary parts alike.
+//
+// All four kernels are PERSISTENT: a CTA walks a contiguous chunk of rows (row blocks), so that
+// everything that depends on the thread only -- twiddles, swizzled shared-memory addresses --
+// is set up once (RowFFT::Ctx, fft.cuh), and the global loads of the next row are issued
+// before the butterflies of the current one.
 #include "hfft_internal.h"
 #include "fft.cuh"
 
 namespace hfft {
 
+// CTA size limit of the x kernels (fp32: 2 CTAs of 512 per SM, i.e. at most 64 registers per thread)
+template <typename T> struct XCfg {
+    static constexpr int MAXT = sizeof(T) == 4 ? 512 : 256;
+    static constexpr int MINB = sizeof(T) == 4 ? 2 : 1;
+};
+
+// first shared-space address >= the dynamic shared memory base that is a multiple of `align`
+__device__ __forceinline__ unsigned smem_base_aligned(unsigned align) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    return (smem_u32(smem_raw) + align - 1) & ~(align - 1);
+}
+
 // ------------------------------------------------------------------------------------------
 // S1: forward x.  A real row of 2N samples (only the first N non-zero if ZP) is packed as N
 // complex z[t] = x[2t] + i x[2t+1]; Z = DFT_N(z); X[k] = E[k] + W_2N^k O[k] with
 // E = (Z[k] + conj Z[N-k]) / 2, O = (Z[k] - conj Z[N-k]) / (2i).
-// One CTA = RB consecutive rows (y) of one plane; the split post-processing runs with lanes
-// along y so that every store to the transposed X^ is a run of RB consecutive elements.
+// One row block = rb consecutive rows (y) of one plane.  Phase 1: thread (r, j) transforms row r.
+// Phase 2: thread (kk, rr) forms the pairs X[k], X[N-k], k = kk + TPR it, of row rr -- lanes run
+// along y so that every store to the transposed X^ is a run of rb consecutive elements.  The
+// element index of row r is XOR-ed with r in shared memory, which makes the phase-2 reads
+// (same k, 16 different rows) conflict free.
 // ------------------------------------------------------------------------------------------
 template <typename T, int LOG2N, bool ZP>
-__global__ void __launch_bounds__(1024)
-fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int rb, int rows_per_plane, int nz, int use_ms,
-                MsParam<T> ms, const HFFT_C* __restrict__ tw /* exp(-2 pi i t / 2N), 2N entries */) {
+__global__ void __launch_bounds__(XCfg<T>::MAXT, XCfg<T>::MINB)
+fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb, int rows_per_plane, int nz,
+                int use_ms, MsParam<T> ms, const HFFT_C* __restrict__ tw /* exp(-2 pi i t / 2N), 2N entries */,
+                const HFFT_C* __restrict__ twt, long long nblocks, int bpc) {
     typedef HFFT_C C;
-    typedef RowFFT<T, LOG2N, false, ZP> F;
-    constexpr int N = F::N, R = F::R, TPR = F::TPR, PITCH = N + 1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C* s = reinterpret_cast<C*>(smem_raw);
-    const int tid = threadIdx.x;
-    const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
-    const long long row0 = (long long)blockIdx.x * rb;          // global row index (plane * rows + y)
-    const int plane = (int)(row0 / rows_per_plane);
-    const int y0 = (int)(row0 - (long long)plane * rows_per_plane);
-    const C* zin = reinterpret_cast<const C*>(in) + (row0 + r) * (ZP ? N / 2 : N);
-    C v[R];
-    constexpr int RL = (ZP && R > 1) ? R / 2 : R;
-#pragma unroll
-    for (int q = 0; q < RL; ++q) v[q] = zin[j + q * TPR];
-    if (ZP && use_ms) {
-        const T sc = ms.v[plane % nz];
-#pragma unroll
-        for (int q = 0; q < RL; ++q) { v[q].x *= sc; v[q].y *= sc; }
-    }
-    C* srow = s + r * PITCH;
-    F::run(v, srow, j, tw, 2);
-    __syncthreads();
-#pragma unroll
-    for (int q = 0; q < R; ++q) srow[swz(j + q * TPR)] = v[q];
-    __syncthreads();
+    typedef RowFFT<T, LOG2N, false, ZP, false> F;
+    constexpr int N = F::N, R = F::R, TPR = F::TPR, SH = F::SH;
+    constexpr int RL = (ZP && R > 1) ? R / 2 : R;            // loads per thread
+    constexpr int IT = R > 1 ? R / 2 : 1;                    // phase-2 iterations: k = kk + TPR it < N / 2
+    constexpr int PZ = F::EXCH & 1;                          // buffer that receives Z (the next free one)
+    const int tid = threadIdx.x, rb = 1 << log2rb;
+    const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);    // phase 1
+    const int rr = tid & (rb - 1), kk = tid >> log2rb;       // phase 2
+    const unsigned base = smem_base_aligned(F::ROW_BYTES);
+    typename F::Ctx c;
+    F::init(c, base + r * F::ROW_BYTES, j, r & 15 & (N - 1), twt);
+    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)(rr & 15 & (N - 1)) << SH) ^ (PZ ? F::BUF_BYTES : 0u);
 
-    // post-process: pairs (k, N-k), k = 0..N/2, lanes along the rb rows
-    C* xp = xhat + (long long)plane * (N + 1) * rows_per_plane + y0;
-    const int nthreads = blockDim.x;
-    for (int w = tid; w < (N / 2 + 1) * rb; w += nthreads) {
-        const int k = w / rb, rr = w - k * rb;
-        const C* sr = s + rr * PITCH;
-        if (k == 0) {
-            C z0 = sr[0];
-            xp[rr] = mk<T>(z0.x + z0.y, 0);
-            xp[(long long)N * rows_per_plane + rr] = mk<T>(z0.x - z0.y, 0);
-        } else {
-            C zk = sr[swz(k)], zn = sr[swz(N - k)];
-            C E = mk<T>((zk.x + zn.x) * (T)0.5, (zk.y - zn.y) * (T)0.5);
-            C O = mk<T>((zk.y + zn.y) * (T)0.5, (zn.x - zk.x) * (T)0.5);
-            C WO = cmul(__ldg(tw + k), O);
-            xp[(long long)k * rows_per_plane + rr] = cadd(E, WO);
-            if (k != N - k) xp[(long long)(N - k) * rows_per_plane + rr] = cconj(csub(E, WO));
+    long long blk = (long long)blockIdx.x * bpc;
+    const int nit = (int)((nblocks - blk < bpc) ? nblocks - blk : bpc);
+    const int bpp = rows_per_plane >> log2rb;                // row blocks per plane
+    long long plane = blk / bpp;
+    int y0 = (int)(blk - plane * bpp) << log2rb;
+    int layer = (int)(plane % nz);
+    const C* zin = reinterpret_cast<const C*>(in) + (blk * rb + r) * (ZP ? N / 2 : N) + j;
+    const long long zstep = (long long)rb * (ZP ? N / 2 : N);
+    C v[R];
+#pragma unroll
+    for (int q = 0; q < RL; ++q) v[q] = zin[q * TPR];
+
+    for (int it0 = 0; it0 < nit; ++it0) {
+        if (ZP && use_ms) {
+            const T sc = ms.v[layer];
+#pragma unroll
+            for (int q = 0; q < RL; ++q) v[q] = cscale(sc, v[q]);
         }
+        F::run(v, c);
+#pragma unroll
+        for (int q = 0; q < R; ++q) sts(F::template elem_addr<PZ>(c, q), v[q]);
+        if (it0 + 1 < nit) {                                 // next block's loads fly during phase 2
+            zin += zstep;
+#pragma unroll
+            for (int q = 0; q < RL; ++q) v[q] = zin[q * TPR];
+        }
+        __syncthreads();
+
+        C* xp = xhat + plane * (long long)(N + 1) * rows_per_plane + y0 + rr;
+#pragma unroll
+        for (int it = 0; it < IT; ++it) {
+            const int k = kk + TPR * it;
+            if (it == 0 && kk == 0) {
+                const C z0 = lds<C>(zrow);
+                xp[0] = mk<T>(z0.x + z0.y, 0);
+                xp[(long long)N * rows_per_plane] = mk<T>(z0.x - z0.y, 0);
+                const C zm = lds<C>(zrow ^ ((unsigned)swz(N / 2) << SH));
+                xp[(long long)(N / 2) * rows_per_plane] = cconj(zm);           // W_2N^{N/2} = -i
+            } else {
+                const C zk = lds<C>(zrow ^ ((unsigned)swz(k) << SH));
+                const C zn = cconj(lds<C>(zrow ^ ((unsigned)swz(N - k) << SH)));
+                const C s = cadd(zk, zn);                                      // 2 E
+                const C wo = cmul(mul_mi(csub(zk, zn)), __ldg(tw + k));        // 2 W O
+                xp[(long long)k * rows_per_plane] = cscale((T)0.5, cadd(s, wo));
+                xp[(long long)(N - k) * rows_per_plane] = cconj(cscale((T)0.5, csub(s, wo)));
+            }
+        }
+        __syncthreads();                                     // Z is consumed before the next block's exchanges
+        y0 += rb;
+        if (y0 == rows_per_plane) { y0 = 0; ++plane; if (++layer == nz) layer = 0; }
     }
 }
 
 // ------------------------------------------------------------------------------------------
 // S5: inverse x (complex-to-real, crop to the first N reals = first N/2 complex outputs).
 // Z~[k] = E~ + i O~,  E~ = X[k] + conj X[N-k],  O~ = (X[k] - conj X[N-k]) W_2N^{-k};
-// z~ = IDFT_N(Z~) holds x~[2t] + i x~[2t+1].  Same CTA shape as S1: the pre-processing reads the
-// transposed X^ with lanes along y.
+// z~ = IDFT_N(Z~) holds x~[2t] + i x~[2t+1].  Same row blocks as S1: phase 1 reads the
+// transposed X^ with lanes along y and writes Z~ to the rows in shared memory, phase 2 is the
+// row transform; only the first half of its outputs is stored (fused crop).
 // ------------------------------------------------------------------------------------------
 template <typename T, int LOG2N>
-__global__ void __launch_bounds__(1024)
-ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int rb, int rows_per_plane,
-             const HFFT_C* __restrict__ tw) {
+__global__ void __launch_bounds__(XCfg<T>::MAXT, XCfg<T>::MINB)
+ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, int rows_per_plane,
+             const HFFT_C* __restrict__ tw, const HFFT_C* __restrict__ twt, long long nblocks, int bpc) {
     typedef HFFT_C C;
-    typedef RowFFT<T, LOG2N, true, false> F;
-    constexpr int N = F::N, R = F::R, TPR = F::TPR, PITCH = N + 1;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C* s = reinterpret_cast<C*>(smem_raw);
-    const int tid = threadIdx.x;
-    const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
-    const long long row0 = (long long)blockIdx.x * rb;
-    const int plane = (int)(row0 / rows_per_plane);
-    const int y0 = (int)(row0 - (long long)plane * rows_per_plane);
-    const C* xp = xhat + (long long)plane * (N + 1) * rows_per_plane + y0;
-    const int nthreads = blockDim.x;
-    for (int w = tid; w < (N / 2 + 1) * rb; w += nthreads) {
-        const int k = w / rb, rr = w - k * rb;
-        C* sr = s + rr * PITCH;
-        C xk = xp[(long long)k * rows_per_plane + rr];
-        C xn = xp[(long long)(N - k) * rows_per_plane + rr];      // k = 0: the Nyquist row kx = N
-        C E = mk<T>(xk.x + xn.x, xk.y - xn.y);
-        C D = mk<T>(xk.x - xn.x, xk.y + xn.y);
-        C O = (k == 0) ? D : cmulc(D, __ldg(tw + k));
-        // Z~[k] = E + i O ; Z~[N-k] = conj(E) + i conj(O)
-        sr[swz(k)] = mk<T>(E.x - O.y, E.y + O.x);
-        if (k != 0 && k != N - k) sr[swz(N - k)] = mk<T>(E.x + O.y, O.x - E.y);
+    typedef RowFFT<T, LOG2N, true, false, false> F;
+    constexpr int N = F::N, R = F::R, TPR = F::TPR, SH = F::SH;
+    constexpr int IT = R > 1 ? R / 2 : 1;
+    constexpr int RS = R > 1 ? R / 2 : 1;                    // stores per thread (crop)
+    constexpr int PZ = 1;                                    // Z~ sits in buffer 1: exchange 0 writes buffer 0
+    const int tid = threadIdx.x, rb = 1 << log2rb;
+    const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);    // phase 2
+    const int rr = tid & (rb - 1), kk = tid >> log2rb;       // phase 1
+    const unsigned base = smem_base_aligned(F::ROW_BYTES);
+    typename F::Ctx c;
+    F::init(c, base + r * F::ROW_BYTES, j, r & 15 & (N - 1), twt);
+    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)(rr & 15 & (N - 1)) << SH) ^ F::BUF_BYTES;
+
+    long long blk = (long long)blockIdx.x * bpc;
+    const int nit = (int)((nblocks - blk < bpc) ? nblocks - blk : bpc);
+    const int bpp = rows_per_plane >> log2rb;
+    long long plane = blk / bpp;
+    int y0 = (int)(blk - plane * bpp) << log2rb;
+    C* zout = reinterpret_cast<C*>(out) + (blk * rb + r) * (N / 2) + j;
+    const long long zstep = (long long)rb * (N / 2);
+
+    for (int it0 = 0; it0 < nit; ++it0) {
+        const C* xp = xhat + plane * (long long)(N + 1) * rows_per_plane + y0 + rr;
+#pragma unroll
+        for (int it = 0; it < IT; ++it) {
+            const int k = kk + TPR * it;
+            if (it == 0 && kk == 0) {
+                const C x0 = xp[0], xn = xp[(long long)N * rows_per_plane];     // DC and Nyquist (both real)
+                const C e = cadd(x0, cconj(xn)), d = csub(x0, cconj(xn));
+                sts(zrow, mk<T>(e.x - d.y, e.y + d.x));
+                const C xm = xp[(long long)(N / 2) * rows_per_plane];
+                sts(zrow ^ ((unsigned)swz(N / 2) << SH), mk<T>(2 * xm.x, -2 * xm.y));
+            } else {
+                const C xk = xp[(long long)k * rows_per_plane];
+                const C xn = cconj(xp[(long long)(N - k) * rows_per_plane]);
+                const C e = cadd(xk, xn);
+                const C o = mul_pi(cmulc(csub(xk, xn), __ldg(tw + k)));        // i O~
+                sts(zrow ^ ((unsigned)swz(k) << SH), cadd(e, o));              // Z~[k] = E~ + i O~
+                sts(zrow ^ ((unsigned)swz(N - k) << SH), cconj(csub(e, o)));   // Z~[N-k] = conj(E~ - i O~)
+            }
+        }
+        __syncthreads();
+        C v[R];
+#pragma unroll
+        for (int q = 0; q < R; ++q) v[q] = lds<C>(F::template elem_addr<PZ>(c, q));
+        F::run(v, c);
+#pragma unroll
+        for (int q = 0; q < RS; ++q) zout[q * TPR] = v[q];
+        zout += zstep;
+        __syncthreads();                                     // rows are free for the next block's Z~
+        y0 += rb;
+        if (y0 == rows_per_plane) { y0 = 0; ++plane; }
     }
-    __syncthreads();
-    C* srow = s + r * PITCH;
-    C v[R];
-#pragma unroll
-    for (int q = 0; q < R; ++q) v[q] = srow[swz(j + q * TPR)];
-    F::run(v, srow, j, tw, 2);
-    C* zout = reinterpret_cast<C*>(out) + (row0 + r) * (N / 2);
-    constexpr int RS = R > 1 ? R / 2 : 1;
-#pragma unroll
-    for (int q = 0; q < RS; ++q) zout[j + q * TPR] = v[q];
 }
 
 // ------------------------------------------------------------------------------------------
 // S2 / S4: transforms along y on the contiguous rows of the transposed X^.  Row = (plane, kx);
-// a CTA handles `rpc` consecutive rows, TPR threads per row.
+// a CTA holds blockDim / TPR rows at a time and walks `gpc` consecutive row groups.
 // ------------------------------------------------------------------------------------------
+template <int LOG2N> struct YCfg {
+    static constexpr int TPR = (1 << LOG2N) / (LOG2N < 3 ? (1 << LOG2N) : 8);
+    static constexpr int THREADS = TPR > 128 ? TPR : 128;
+};
+
+// (plane, kx) of a row and whether the plane is a z component (nz_rot layers per component)
+struct RowPos {
+    long long plane; int kx; int pl3;
+    __device__ __forceinline__ void set(long long row, int nxp1, int nz_rot) {
+        plane = row / nxp1; kx = (int)(row - plane * nxp1);
+        pl3 = nz_rot > 0 ? (int)(plane % (3 * nz_rot)) : 0;
+    }
+    __device__ __forceinline__ void advance(int rows, int nxp1, int nz_rot) {
+        kx += rows;
+        while (kx >= nxp1) { kx -= nxp1; ++plane; if (++pl3 == 3 * nz_rot) pl3 = 0; }
+    }
+    __device__ __forceinline__ bool is_z(int nz_rot) const { return nz_rot > 0 && pl3 >= 2 * nz_rot; }
+};
+
 template <typename T, int LOG2N, bool ZP>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(YCfg<LOG2N>::THREADS)
 ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long long nrows, int nxp1, int nz_rot,
-                long long ks, const HFFT_C* __restrict__ tw /* N entries */) {
+                long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc) {
     typedef HFFT_C C;
-    typedef RowFFT<T, LOG2N, false, ZP> F;
+    typedef RowFFT<T, LOG2N, false, ZP, sizeof(T) == 4> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C* s = reinterpret_cast<C*>(smem_raw);
+    constexpr int RL = ZP ? R / 2 : R;
     const int tid = threadIdx.x;
     const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
     const int rpc = blockDim.x >> F::LOG2TPR;
-    const long long row = (long long)blockIdx.x * rpc + r;
-    const bool live = row < nrows;
-    const long long rowc = live ? row : nrows - 1;
-    const C* zin = xhat + rowc * (ZP ? N / 2 : N);
-    C v[R];
-    constexpr int RL = ZP ? R / 2 : R;
+    typename F::Ctx c;
+    F::init(c, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
+
+    const long long g0 = (long long)blockIdx.x * gpc;
+    const int nit = (int)((ngroups - g0 < gpc) ? ngroups - g0 : gpc);
+    long long row = g0 * rpc + r;
+    RowPos pos; pos.set(row < nrows ? row : nrows - 1, nxp1, nz_rot);
+    const C* zin = xhat + row * (ZP ? N / 2 : N) + j;
+    const long long zstep = (long long)rpc * (ZP ? N / 2 : N);
+    C nv[RL];
+    bool live = row < nrows;
+    if (live) {
 #pragma unroll
-    for (int q = 0; q < RL; ++q) v[q] = zin[j + q * TPR];
-    F::run(v, s + r * N, j, tw, 1);
-    if (!live) return;
-    const int plane = (int)(row / nxp1);
-    const int kx = (int)(row - (long long)plane * nxp1);
-    if (nz_rot > 0 && (plane / nz_rot) % 3 == 2) {   // M'_z = i M_z
-#pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = mul_pi(v[q]);
+        for (int q = 0; q < RL; ++q) nv[q] = zin[q * TPR];
     }
-    C* dst = spec + (long long)plane * ks + (long long)kx * N;
+    for (int it = 0; it < nit; ++it) {
+        C v[R];
 #pragma unroll
-    for (int q = 0; q < R; ++q) dst[j + q * TPR] = v[q];
+        for (int q = 0; q < RL; ++q) v[q] = nv[q];
+        const bool cur_live = live;
+        const bool rot = pos.is_z(nz_rot);
+        C* dst = spec + pos.plane * ks + (long long)pos.kx * N + j;
+        row += rpc; zin += zstep;
+        live = (it + 1 < nit) && row < nrows;
+        if (live) {
+            pos.advance(rpc, nxp1, nz_rot);
+#pragma unroll
+            for (int q = 0; q < RL; ++q) nv[q] = zin[q * TPR];
+        }
+        F::run(v, c);
+        if (cur_live) {
+            if (rot) {                                       // M'_z = i M_z
+#pragma unroll
+                for (int q = 0; q < R; ++q) v[q] = mul_pi(v[q]);
+            }
+#pragma unroll
+            for (int q = 0; q < R; ++q) dst[q * TPR] = v[q];
+        }
+    }
 }
 
 template <typename T, int LOG2N>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(YCfg<LOG2N>::THREADS)
 iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long long nrows, int nxp1, int nz_rot,
-             long long ks, const HFFT_C* __restrict__ tw) {
+             long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc) {
     typedef HFFT_C C;
-    typedef RowFFT<T, LOG2N, true, false> F;
+    typedef RowFFT<T, LOG2N, true, false, sizeof(T) == 4> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    C* s = reinterpret_cast<C*>(smem_raw);
     const int tid = threadIdx.x;
     const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
     const int rpc = blockDim.x >> F::LOG2TPR;
-    const long long row = (long long)blockIdx.x * rpc + r;
-    const bool live = row < nrows;
-    const long long rowc = live ? row : nrows - 1;
-    const int plane = (int)(rowc / nxp1);
-    const int kx = (int)(rowc - (long long)plane * nxp1);
-    const C* src = spec + (long long)plane * ks + (long long)kx * N;
-    C v[R];
+    typename F::Ctx c;
+    F::init(c, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
+
+    const long long g0 = (long long)blockIdx.x * gpc;
+    const int nit = (int)((ngroups - g0 < gpc) ? ngroups - g0 : gpc);
+    long long row = g0 * rpc + r;
+    RowPos pos; pos.set(row < nrows ? row : nrows - 1, nxp1, nz_rot);
+    C nv[R];
+    bool live = row < nrows;
+    if (live) {
+        const C* src = spec + pos.plane * ks + (long long)pos.kx * N + j;
 #pragma unroll
-    for (int q = 0; q < R; ++q) v[q] = src[j + q * TPR];
-    if (nz_rot > 0 && (plane / nz_rot) % 3 == 2) {   // H_z = -i H'_z
-#pragma unroll
-        for (int q = 0; q < R; ++q) v[q] = mul_mi(v[q]);
+        for (int q = 0; q < R; ++q) nv[q] = src[q * TPR];
     }
-    F::run(v, s + r * N, j, tw, 1);
-    if (!live) return;
-    C* dst = xhat + row * (N / 2);
+    for (int it = 0; it < nit; ++it) {
+        C v[R];
+        const bool cur_live = live;
+        const bool rot = pos.is_z(nz_rot);
 #pragma unroll
-    for (int q = 0; q < R / 2; ++q) dst[j + q * TPR] = v[q];
+        for (int q = 0; q < R; ++q) v[q] = rot ? mul_mi(nv[q]) : nv[q];        // H_z = -i H'_z
+        C* dst = xhat + row * (N / 2) + j;
+        row += rpc;
+        live = (it + 1 < nit) && row < nrows;
+        if (live) {
+            pos.advance(rpc, nxp1, nz_rot);
+            const C* src = spec + pos.plane * ks + (long long)pos.kx * N + j;
+#pragma unroll
+            for (int q = 0; q < R; ++q) nv[q] = src[q * TPR];
+        }
+        F::run(v, c);
+        if (cur_live) {
+#pragma unroll
+            for (int q = 0; q < R / 2; ++q) dst[q * TPR] = v[q];
+        }
+    }
 }
 
 // ------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------
-// opt in to > 48 KB of dynamic shared memory once per kernel instantiation (`done` is a static
-// local of the dispatch case, i.e. one flag per instantiation)
-template <typename K> static cudaError_t set_smem(K kernel, size_t bytes, size_t& done) {
-    if (bytes <= 48 * 1024 || bytes <= done) return cudaSuccess;
-    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-    if (e == cudaSuccess) done = bytes;
-    return e;
+// Per kernel instantiation: opt in to > 48 KB of dynamic shared memory and ask the runtime how
+// many CTAs fit an SM (cached for the last (threads, smem) pair; `Tag` makes one cache per case).
+struct LaunchCache { int threads = 0; size_t smem = 0, smem_opt = 0; int occ = 0; };
+template <typename K>
+static cudaError_t ctas_per_sm(K kernel, int threads, size_t smem, LaunchCache& lc, int& occ) {
+    cudaError_t e;
+    if (smem > 48 * 1024 && smem > lc.smem_opt) {
+        if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
+        lc.smem_opt = smem;
+    }
+    if (lc.threads != threads || lc.smem != smem) {
+        int nb = 0;
+        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, smem)) != cudaSuccess) return e;
+        lc.threads = threads; lc.smem = smem; lc.occ = nb < 1 ? 1 : nb;
+    }
+    occ = lc.occ;
+    return cudaSuccess;
+}
+
+// persistent grid: `items` units of work in contiguous chunks of `per_cta`
+static void chunk_grid(long long items, int num_sms, int occ, unsigned& grid, int& per_cta) {
+    long long g = (long long)num_sms * occ;
+    if (g > items) g = items;
+    if (g < 1) g = 1;
+    long long pc = (items + g - 1) / g;
+    grid = (unsigned)((items + pc - 1) / pc);
+    per_cta = (int)pc;
 }
 
 #define HFFT_CASE(V, ...) case V: { constexpr int L = V; __VA_ARGS__ } break;
@@ -221,35 +355,42 @@ template <typename K> static cudaError_t set_smem(K kernel, size_t bytes, size_t
         default: break;                                                                             \
     }
 
-// rows per CTA of the x kernels: a 128-byte run of the transposed X^, at most 1024 threads
-template <typename T> static int x_rows_per_cta(int log2N, int rows_per_plane) {
-    const int tpr = (1 << log2N) / (log2N < 3 ? (1 << log2N) : 8);
+static int fft_tpr(int log2N) { return (1 << log2N) / (log2N < 3 ? (1 << log2N) : 8); }
+
+// rows per block of the x kernels: a 128-byte run of the transposed X^, at most XCfg::MAXT threads
+template <typename T> static int x_log2_rows_per_block(int log2N, int rows_per_plane) {
+    const int tpr = fft_tpr(log2N);
     int rb = (int)(128 / sizeof(HFFT_C));
-    while (rb > 1 && rb * tpr > 1024) rb /= 2;
-    if (rb > rows_per_plane) rb = rows_per_plane;
-    return rb;
+    while (rb > 1 && rb * tpr > XCfg<T>::MAXT) rb /= 2;
+    while (rb > rows_per_plane) rb /= 2;
+    int l = 0;
+    while ((1 << l) < rb) ++l;
+    return l;
 }
 
 template <typename T, bool ZP>
 cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, int rows_per_plane, int nz,
-                            const double* ms_host, const void* tw, cudaStream_t st) {
+                            const double* ms_host, const void* tw, const void* twt, int num_sms, cudaStream_t st) {
     typedef HFFT_C C;
     const int N = 1 << log2nx;
-    const int rb = x_rows_per_cta<T>(log2nx, rows_per_plane);
-    const int tpr = N / (log2nx < 3 ? N : 8);
-    const size_t smem = (size_t)rb * (N + 1) * sizeof(C);
-    const long long grid = (long long)nplanes * rows_per_plane / rb;
+    const int log2rb = x_log2_rows_per_block<T>(log2nx, rows_per_plane), rb = 1 << log2rb;
+    const int threads = rb * fft_tpr(log2nx);
+    const size_t row_bytes = (size_t)2 * N * sizeof(C);
+    const size_t smem = (rb + 1) * row_bytes;
+    const long long nblocks = (long long)nplanes * rows_per_plane / rb;
     MsParam<T> ms;
     const int use_ms = ms_host != nullptr;
     for (int k = 0; k < HFFT_MAX_NZ; ++k) ms.v[k] = (use_ms && k < nz) ? (T)ms_host[k] : (T)1;
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_X(log2nx, {
         auto kern = fftx_fwd_kernel<T, L, ZP>;
-        static size_t smem_done = 0;
-        err = set_smem(kern, smem, smem_done);
-        if (err == cudaSuccess) {
-            kern<<<(unsigned)grid, rb * tpr, smem, st>>>(in, (C*)xhat, rb, rows_per_plane, nz > 0 ? nz : 1, use_ms, ms,
-                                                         (const C*)tw);
+        static LaunchCache lc;
+        int occ = 1;
+        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+            unsigned grid; int bpc;
+            chunk_grid(nblocks, num_sms, occ, grid, bpc);
+            kern<<<grid, threads, smem, st>>>(in, (C*)xhat, log2rb, rows_per_plane, nz > 0 ? nz : 1, use_ms, ms,
+                                              (const C*)tw, (const C*)twt, nblocks, bpc);
             err = cudaGetLastError();
         }
     })
@@ -258,20 +399,24 @@ cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, in
 
 template <typename T>
 cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw,
-                         cudaStream_t st) {
+                         const void* twt, int num_sms, cudaStream_t st) {
     typedef HFFT_C C;
     const int N = 1 << log2nx;
-    const int rb = x_rows_per_cta<T>(log2nx, rows_per_plane);
-    const int tpr = N / (log2nx < 3 ? N : 8);
-    const size_t smem = (size_t)rb * (N + 1) * sizeof(C);
-    const long long grid = (long long)nplanes * rows_per_plane / rb;
+    const int log2rb = x_log2_rows_per_block<T>(log2nx, rows_per_plane), rb = 1 << log2rb;
+    const int threads = rb * fft_tpr(log2nx);
+    const size_t row_bytes = (size_t)2 * N * sizeof(C);
+    const size_t smem = (rb + 1) * row_bytes;
+    const long long nblocks = (long long)nplanes * rows_per_plane / rb;
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_X(log2nx, {
         auto kern = ifftx_kernel<T, L>;
-        static size_t smem_done = 0;
-        err = set_smem(kern, smem, smem_done);
-        if (err == cudaSuccess) {
-            kern<<<(unsigned)grid, rb * tpr, smem, st>>>((const C*)xhat, out, rb, rows_per_plane, (const C*)tw);
+        static LaunchCache lc;
+        int occ = 1;
+        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+            unsigned grid; int bpc;
+            chunk_grid(nblocks, num_sms, occ, grid, bpc);
+            kern<<<grid, threads, smem, st>>>((const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
+                                              (const C*)twt, nblocks, bpc);
             err = cudaGetLastError();
         }
     })
@@ -280,22 +425,26 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
 
 template <typename T, bool ZP>
 cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                            const void* tw, cudaStream_t st) {
+                            const void* twt, int num_sms, cudaStream_t st) {
     typedef HFFT_C C;
     const int N = 1 << log2N;
-    const int tpr = log2N < 3 ? 1 : N / 8;
-    const int rpc = tpr >= 256 ? 1 : 256 / tpr;
+    const int tpr = fft_tpr(log2N);
+    const int threads = tpr > 128 ? tpr : 128;
+    const int rpc = threads / tpr;
     const long long nrows = (long long)nplanes * (nx + 1);
-    const size_t smem = (size_t)rpc * N * sizeof(C);
-    const long long grid = (nrows + rpc - 1) / rpc;
+    const size_t row_bytes = (size_t)2 * N * sizeof(C);
+    const size_t smem = (rpc + 1) * row_bytes;
+    const long long ngroups = (nrows + rpc - 1) / rpc;
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_Y(log2N, {
         auto kern = ffty_fwd_kernel<T, L, ZP>;
-        static size_t smem_done = 0;
-        err = set_smem(kern, smem, smem_done);
-        if (err == cudaSuccess) {
-            kern<<<(unsigned)grid, rpc * tpr, smem, st>>>((const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks,
-                                                          (const C*)tw);
+        static LaunchCache lc;
+        int occ = 1;
+        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+            unsigned grid; int gpc;
+            chunk_grid(ngroups, num_sms, occ, grid, gpc);
+            kern<<<grid, threads, smem, st>>>((const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks, (const C*)twt,
+                                              ngroups, gpc);
             err = cudaGetLastError();
         }
     })
@@ -304,22 +453,26 @@ cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int
 
 template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                         const void* tw, cudaStream_t st) {
+                         const void* twt, int num_sms, cudaStream_t st) {
     typedef HFFT_C C;
     const int N = 1 << log2N;
-    const int tpr = log2N < 3 ? 1 : N / 8;
-    const int rpc = tpr >= 256 ? 1 : 256 / tpr;
+    const int tpr = fft_tpr(log2N);
+    const int threads = tpr > 128 ? tpr : 128;
+    const int rpc = threads / tpr;
     const long long nrows = (long long)nplanes * (nx + 1);
-    const size_t smem = (size_t)rpc * N * sizeof(C);
-    const long long grid = (nrows + rpc - 1) / rpc;
+    const size_t row_bytes = (size_t)2 * N * sizeof(C);
+    const size_t smem = (rpc + 1) * row_bytes;
+    const long long ngroups = (nrows + rpc - 1) / rpc;
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_Y(log2N, {
         auto kern = iffty_kernel<T, L>;
-        static size_t smem_done = 0;
-        err = set_smem(kern, smem, smem_done);
-        if (err == cudaSuccess) {
-            kern<<<(unsigned)grid, rpc * tpr, smem, st>>>((const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks,
-                                                          (const C*)tw);
+        static LaunchCache lc;
+        int occ = 1;
+        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+            unsigned grid; int gpc;
+            chunk_grid(ngroups, num_sms, occ, grid, gpc);
+            kern<<<grid, threads, smem, st>>>((const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks, (const C*)twt,
+                                              ngroups, gpc);
             err = cudaGetLastError();
         }
     })
@@ -327,15 +480,15 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
 }
 
 // explicit instantiations used by hfft_api.cu / tensor_build.cu
-template cudaError_t launch_fftx_fwd<float, true>(const float*, void*, int, int, int, int, const double*, const void*, cudaStream_t);
-template cudaError_t launch_fftx_fwd<double, true>(const double*, void*, int, int, int, int, const double*, const void*, cudaStream_t);
-template cudaError_t launch_fftx_fwd<double, false>(const double*, void*, int, int, int, int, const double*, const void*, cudaStream_t);
-template cudaError_t launch_ifftx<float>(const void*, float*, int, int, int, const void*, cudaStream_t);
-template cudaError_t launch_ifftx<double>(const void*, double*, int, int, int, const void*, cudaStream_t);
-template cudaError_t launch_ffty_fwd<float, true>(const void*, void*, int, int, int, int, long long, const void*, cudaStream_t);
-template cudaError_t launch_ffty_fwd<double, true>(const void*, void*, int, int, int, int, long long, const void*, cudaStream_t);
-template cudaError_t launch_ffty_fwd<double, false>(const void*, void*, int, int, int, int, long long, const void*, cudaStream_t);
-template cudaError_t launch_iffty<float>(const void*, void*, int, int, int, int, long long, const void*, cudaStream_t);
-template cudaError_t launch_iffty<double>(const void*, void*, int, int, int, int, long long, const void*, cudaStream_t);
+template cudaError_t launch_fftx_fwd<float, true>(const float*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_fftx_fwd<double, true>(const double*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_fftx_fwd<double, false>(const double*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_ifftx<float>(const void*, float*, int, int, int, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_ifftx<double>(const void*, double*, int, int, int, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_ffty_fwd<float, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
+template cudaError_t launch_ffty_fwd<double, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
+template cudaError_t launch_ffty_fwd<double, false>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
+template cudaError_t launch_iffty<float>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
+template cudaError_t launch_iffty<double>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
 
 }  // namespace hfft

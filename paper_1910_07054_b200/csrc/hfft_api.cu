@@ -27,8 +27,10 @@ struct hfft_plan {
     size_t ws_xhat = 0, ws_spec = 0, ws_stage_m = 0, ws_stage_h = 0;   // offsets into the workspace
     void *bank = nullptr, *ws = nullptr;
     bool own_bank = false, own_ws = false, built = false;
-    void *tw_x = nullptr, *tw_y = nullptr;           // plan precision, 2nx and 2ny entries
-    void *tw_x64 = nullptr, *tw_y64 = nullptr;       // fp64 (setup); alias tw_x/tw_y for an fp64 plan
+    // tw_x: exp(-2 pi i t / 2nx), 2nx entries; twt_x / twt_y: per-thread tables of the length-nx and
+    // length-2ny row transforms (fft.cuh).  *64: fp64 copies for the setup (aliases for an fp64 plan).
+    void *tw_x = nullptr, *twt_x = nullptr, *twt_y = nullptr;
+    void *tw_x64 = nullptr, *twt_x64 = nullptr, *twt_y64 = nullptr;
     bool profiling = false;
     int prof_calls = 0;
     std::vector<cudaEvent_t> prof_events;            // (HFFT_NUM_STAGES + 1) per call
@@ -76,20 +78,52 @@ static void twiddle_table(int N, std::vector<double>& re, std::vector<double>& i
     }
 }
 
-static cudaError_t upload_twiddles(int N, bool f32, void** out) {
-    std::vector<double> re, im;
-    twiddle_table(N, re, im);
+// Per-thread twiddle table of the length-2^log2N row transform, in the order the kernels consume it
+// (fft.cuh, RowFFT): stages after the first; radix 2^lr, U = R / radix butterflies per thread;
+// slot (stage, u, t) holds, for thread j < TPR, exp(-2 pi i t k / (N_s radix)), k = (j + u TPR) mod N_s.
+static void thread_twiddle_table(int log2N, std::vector<double>& re, std::vector<double>& im) {
+    const int N = 1 << log2N, log2R = log2N < 3 ? log2N : 3, R = 1 << log2R, TPR = N / R;
+    std::vector<double> tr, ti;
+    twiddle_table(N, tr, ti);
+    re.clear(); im.clear();
+    for (int lns = log2R; lns < log2N;) {
+        const int lr = (log2N - lns >= 3) ? 3 : log2N - lns;
+        const int rad = 1 << lr, U = R / rad, NS = 1 << lns;
+        for (int u = 0; u < U; ++u)
+            for (int t = 1; t < rad; ++t)
+                for (int j = 0; j < TPR; ++j) {
+                    const long long k = (j + u * TPR) & (NS - 1);
+                    const long long idx = (t * k * (N >> (lns + lr))) % N;
+                    re.push_back(tr[idx]); im.push_back(ti[idx]);
+                }
+        lns += lr;
+    }
+    if (re.empty()) { re.push_back(1.0); im.push_back(0.0); }   // single-stage transforms read nothing
+}
+
+static cudaError_t upload_complex(const std::vector<double>& re, const std::vector<double>& im, bool f32, void** out) {
+    const size_t n = re.size();
     cudaError_t e;
     if (f32) {
-        std::vector<float> h(2 * (size_t)N);
-        for (int t = 0; t < N; ++t) { h[2 * t] = (float)re[t]; h[2 * t + 1] = (float)im[t]; }
+        std::vector<float> h(2 * n);
+        for (size_t t = 0; t < n; ++t) { h[2 * t] = (float)re[t]; h[2 * t + 1] = (float)im[t]; }
         if ((e = cudaMalloc(out, h.size() * sizeof(float))) != cudaSuccess) return e;
         return cudaMemcpy(*out, h.data(), h.size() * sizeof(float), cudaMemcpyHostToDevice);
     }
-    std::vector<double> h(2 * (size_t)N);
-    for (int t = 0; t < N; ++t) { h[2 * t] = re[t]; h[2 * t + 1] = im[t]; }
+    std::vector<double> h(2 * n);
+    for (size_t t = 0; t < n; ++t) { h[2 * t] = re[t]; h[2 * t + 1] = im[t]; }
     if ((e = cudaMalloc(out, h.size() * sizeof(double))) != cudaSuccess) return e;
     return cudaMemcpy(*out, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice);
+}
+static cudaError_t upload_twiddles(int N, bool f32, void** out) {
+    std::vector<double> re, im;
+    twiddle_table(N, re, im);
+    return upload_complex(re, im, f32, out);
+}
+static cudaError_t upload_thread_twiddles(int log2N, bool f32, void** out) {
+    std::vector<double> re, im;
+    thread_twiddle_table(log2N, re, im);
+    return upload_complex(re, im, f32, out);
 }
 
 static void plan_sizes(hfft_plan* p) {
@@ -178,7 +212,7 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->n_k = plan->n_k; info->n_k_padded = plan->n_k_padded;
     info->bank_bytes = plan->bank_bytes; info->workspace_bytes = plan->ws_bytes;
     BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
-                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec};
+                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
     info->setup_scratch_bytes = build_scratch_bytes(g);
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
@@ -214,22 +248,24 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     if ((e = cudaMemsetAsync(plan->ws, 0, plan->ws_bytes, st)) != cudaSuccess) return fail_cuda(plan, "cudaMemsetAsync", e);
     if (!plan->tw_x64) {
         if ((e = upload_twiddles(2 * plan->nx, false, &plan->tw_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if ((e = upload_twiddles(2 * plan->ny, false, &plan->tw_y64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if ((e = upload_thread_twiddles(plan->log2nx, false, &plan->twt_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if ((e = upload_thread_twiddles(plan->log2ny + 1, false, &plan->twt_y64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
         if (plan->prec == HFFT_F32) {
             if ((e = upload_twiddles(2 * plan->nx, true, &plan->tw_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-            if ((e = upload_twiddles(2 * plan->ny, true, &plan->tw_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+            if ((e = upload_thread_twiddles(plan->log2nx, true, &plan->twt_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+            if ((e = upload_thread_twiddles(plan->log2ny + 1, true, &plan->twt_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
         } else {
-            plan->tw_x = plan->tw_x64; plan->tw_y = plan->tw_y64;
+            plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
         }
     }
     BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
-                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec};
+                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
     void* scratch = nullptr;
     const size_t sb = build_scratch_bytes(g);
     if ((e = cudaMalloc(&scratch, sb)) != cudaSuccess)
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
     std::string msg;
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->tw_y64, st, msg);
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, st, msg);
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
     if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_build_tensor: " + msg);
@@ -255,11 +291,13 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
 #define STAGE(idx, call)                                                            \
     if (ev && (e = cudaEventRecord(ev[idx], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e); \
     if ((e = (call)) != cudaSuccess) return fail_cuda(p, #call, e);
-    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, st)))
-    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
+    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, p->twt_x,
+                                       p->num_sms, st)))
+    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y,
+                                       p->num_sms, st)))
     STAGE(2, (launch_coupling<T>(p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded, p->num_sms, st)))
-    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->tw_y, st)))
-    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, st)))
+    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y, p->num_sms, st)))
+    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, st)))
 #undef STAGE
     if (ev) {
         if ((e = cudaEventRecord(ev[HFFT_NUM_STAGES], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);
@@ -358,10 +396,8 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (!plan) return HFFT_OK;
     if (plan->own_bank && plan->bank) cudaFree(plan->bank);
     if (plan->own_ws && plan->ws) cudaFree(plan->ws);
-    if (plan->tw_x && plan->tw_x != plan->tw_x64) cudaFree(plan->tw_x);
-    if (plan->tw_y && plan->tw_y != plan->tw_y64) cudaFree(plan->tw_y);
-    if (plan->tw_x64) cudaFree(plan->tw_x64);
-    if (plan->tw_y64) cudaFree(plan->tw_y64);
+    if (plan->tw_x != plan->tw_x64) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
+    cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
     for (auto& ev : plan->prof_events) cudaEventDestroy(ev);
     delete plan;
     return HFFT_OK;

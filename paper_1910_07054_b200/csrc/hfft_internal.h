@@ -14,21 +14,24 @@ namespace hfft {
 template <typename T> struct MsParam { T v[HFFT_MAX_NZ]; };
 
 // ---- fft_kernels.cu ----
+// tw2nx: exp(-2 pi i t / 2nx), 2nx entries (split / merge of the packed real transform);
+// twt_*: per-thread twiddle table of the row transform (layout in fft.cuh; host: thread_twiddle_table)
 // forward x: `in` real rows [nplanes][rows_per_plane][nx if ZP else 2nx] -> X^ [nplanes][nx+1][rows_per_plane]
 template <typename T, bool ZP>
 cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, int rows_per_plane, int nz,
-                            const double* ms_host, const void* tw2nx, cudaStream_t st);
+                            const double* ms_host, const void* tw2nx, const void* twt_nx, int num_sms,
+                            cudaStream_t st);
 template <typename T>
 cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw2nx,
-                         cudaStream_t st);
+                         const void* twt_nx, int num_sms, cudaStream_t st);
 // forward y: X^ rows [nplanes * (nx+1)][N/2 if ZP else N] -> k side [nplanes][ks], k = kx * N + ky;
 // nz_rot > 0 multiplies the z-component planes by i
 template <typename T, bool ZP>
 cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                            const void* twN, cudaStream_t st);
+                            const void* twt_N, int num_sms, cudaStream_t st);
 template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                         const void* twN, cudaStream_t st);
+                         const void* twt_N, int num_sms, cudaStream_t st);
 
 // ---- coupling.cu ----
 // H^ = bank * M^ in place on the k side.  bank layout [tile][i][j][6][tile_k].
@@ -47,10 +50,12 @@ struct BuildGeom {
     int tile_k;
     long long n_k, n_k_padded;
     int prec;              // hfft_precision
+    int num_sms;
 };
 size_t build_scratch_bytes(const BuildGeom& g);
-// fills `bank` (plan precision); tw2nx_f64 / tw2ny_f64 are fp64 twiddle tables on device
-cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx_f64, const void* tw2ny_f64,
-                       cudaStream_t st, std::string& err);
+// fills `bank` (plan precision); fp64 tables on device: tw2nx (2nx entries) and the per-thread
+// tables of the length-nx and length-2ny row transforms
+cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx_f64, const void* twt_nx_f64,
+                       const void* twt_2ny_f64, cudaStream_t st, std::string& err);
 
 }  // namespace hfft

@@ -170,8 +170,8 @@ size_t build_scratch_bytes(const BuildGeom& g) { return scratch_layout(g).total;
         }                                                                              \
     } while (0)
 
-cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx, const void* tw2ny,
-                       cudaStream_t st, std::string& err) {
+cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx, const void* twt_nx,
+                       const void* twt_2ny, cudaStream_t st, std::string& err) {
     const ScratchLayout L = scratch_layout(g);
     unsigned char* base = static_cast<unsigned char*>(scratch);
     double2* d_zeta = reinterpret_cast<double2*>(base + L.zeta);
@@ -216,8 +216,10 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
             assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
                                                   make_double2(coef.hi, coef.lo));
             HFFT_CK(cudaGetLastError());
-            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, g.log2nx, jn * 6, 2 * ny, 0, nullptr, tw2nx, st)));
-            HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, tw2ny, st)));
+            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, g.log2nx, jn * 6, 2 * ny, 0, nullptr, tw2nx, twt_nx,
+                                                    g.num_sms, st)));
+            HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, twt_2ny, g.num_sms,
+                                                    st)));
             dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
             if (g.prec == HFFT_F32)
                 pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, jn, g.tile_k, g.n_k,
