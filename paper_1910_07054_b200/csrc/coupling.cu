@@ -144,7 +144,9 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
 // ONCE and kept in registers: a warp owns target layer i, a lane owns one wavevector and holds
 // the 6 nz reals a^c_ij(k) of its (i, k) for all source layers j.  The states stream through a
 // STAGES-deep cp.async ring of M^ tiles in shared memory ([3 nz][32] complex each); per state a
-// thread does 18 nz FMAs into 6 accumulators and writes H^ of its (i, k) in place.
+// thread does 18 nz FMAs per owned layer and writes H^ of its (i, k) in place.  A thread owns
+// IPT = 2 target layers when the registers allow (nz <= 8 in fp32): M^ is then read from shared
+// memory once for both (ncu: the one-layer version is shared-memory-bandwidth bound).
 // Tile = 32 wavevectors (hfft_api.cu picks tile_k = 32 when this kernel applies).
 // ------------------------------------------------------------------------------------------
 template <int N> __device__ __forceinline__ void cp_async_wait_group() {
@@ -152,17 +154,18 @@ template <int N> __device__ __forceinline__ void cp_async_wait_group() {
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
 
-template <typename T, int NZ, int STAGES>
-__global__ void __launch_bounds__(32 * NZ)
+template <typename T, int NZ, int IPT, int STAGES>
+__global__ void __launch_bounds__(32 * ((NZ + IPT - 1) / IPT))
 coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int batch, long long n_tiles,
                         long long ks) {
     typedef HFFT_C C;
     constexpr int TK = 32, NP = 3 * NZ;
+    constexpr int NW = (NZ + IPT - 1) / IPT;              // warps; warp w owns target layers w, w + NW, ...
     constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk
     constexpr int CPP = TK / CHUNK_C;                     // chunks per plane row
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* sm = reinterpret_cast<C*>(smem_raw);               // [STAGES][NP][TK]
-    const int tid = threadIdx.x, lane = tid & 31, i = tid >> 5;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         C* sp = spec + tile * TK;
@@ -170,8 +173,8 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
             if (b < batch) {
                 C* dst = sm + (b % STAGES) * (NP * TK);
                 const C* src = sp + (long long)b * NP * ks;
-                for (int w = tid; w < NP * CPP; w += 32 * NZ) {
-                    const int lp = w / CPP, ch = w - lp * CPP;
+                for (int x = tid; x < NP * CPP; x += 32 * NW) {
+                    const int lp = x / CPP, ch = x - lp * CPP;
                     cp_async16(dst + lp * TK + ch * CHUNK_C, src + (long long)lp * ks + ch * CHUNK_C);
                 }
             }
@@ -180,30 +183,47 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
 #pragma unroll
         for (int s = 0; s < STAGES - 1; ++s) issue(s);
 
-        T a[NZ][6];
-        const T* bt = bank + ((tile * NZ + i) * NZ) * (6LL * TK) + lane;
+        T a[IPT][NZ][6];
 #pragma unroll
-        for (int j = 0; j < NZ; ++j)
+        for (int p = 0; p < IPT; ++p) {
+            const int i = w + p * NW;
+            if (i < NZ) {
+                const T* bt = bank + ((tile * NZ + i) * NZ) * (6LL * TK) + lane;
 #pragma unroll
-            for (int c = 0; c < 6; ++c) a[j][c] = __ldcs(bt + (j * 6 + c) * TK);
+                for (int j = 0; j < NZ; ++j)
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) a[p][j][c] = __ldcs(bt + (j * 6 + c) * TK);
+            }
+        }
 
         for (int b = 0; b < batch; ++b) {
             issue(b + STAGES - 1);
             cp_async_wait_group<STAGES - 1>();
             __syncthreads();
             const C* st = sm + (b % STAGES) * (NP * TK) + lane;
-            C hx = mk<T>((T)0, (T)0), hy = hx, hz = hx;
+            C hx[IPT], hy[IPT], hz[IPT];
+#pragma unroll
+            for (int p = 0; p < IPT; ++p) hx[p] = hy[p] = hz[p] = mk<T>((T)0, (T)0);
 #pragma unroll
             for (int j = 0; j < NZ; ++j) {
                 const C mx = st[(0 * NZ + j) * TK], my = st[(1 * NZ + j) * TK], mz = st[(2 * NZ + j) * TK];
-                hx = caxpy(a[j][0], mx, hx); hx = caxpy(a[j][3], my, hx); hx = caxpy(a[j][4], mz, hx);
-                hy = caxpy(a[j][3], mx, hy); hy = caxpy(a[j][1], my, hy); hy = caxpy(a[j][5], mz, hy);
-                hz = caxpy(a[j][2], mz, hz); hz = caxpy(-a[j][4], mx, hz); hz = caxpy(-a[j][5], my, hz);
+#pragma unroll
+                for (int p = 0; p < IPT; ++p) {
+                    hx[p] = caxpy(a[p][j][0], mx, hx[p]); hx[p] = caxpy(a[p][j][3], my, hx[p]); hx[p] = caxpy(a[p][j][4], mz, hx[p]);
+                    hy[p] = caxpy(a[p][j][3], mx, hy[p]); hy[p] = caxpy(a[p][j][1], my, hy[p]); hy[p] = caxpy(a[p][j][5], mz, hy[p]);
+                    hz[p] = caxpy(a[p][j][2], mz, hz[p]); hz[p] = caxpy(-a[p][j][4], mx, hz[p]); hz[p] = caxpy(-a[p][j][5], my, hz[p]);
+                }
             }
             C* o = sp + (long long)b * NP * ks + lane;
-            o[(long long)(0 * NZ + i) * ks] = hx;
-            o[(long long)(1 * NZ + i) * ks] = hy;
-            o[(long long)(2 * NZ + i) * ks] = hz;
+#pragma unroll
+            for (int p = 0; p < IPT; ++p) {
+                const int i = w + p * NW;
+                if (i < NZ) {
+                    o[(long long)(0 * NZ + i) * ks] = hx[p];
+                    o[(long long)(1 * NZ + i) * ks] = hy[p];
+                    o[(long long)(2 * NZ + i) * ks] = hz[p];
+                }
+            }
             __syncthreads();   // every warp is done with this stage before it is refilled
         }
         cp_async_wait_group<0>();
@@ -220,7 +240,11 @@ static cudaError_t launch_coupling_batched_nz(const void* bank, void* spec, int 
                                               long long ks, int num_sms, cudaStream_t st) {
     typedef HFFT_C C;
     constexpr int STAGES = 4;
-    auto kern = coupling_batched_kernel<T, NZ, STAGES>;
+    // two target layers per thread (M^ read from shared memory once for both) while the bank
+    // registers stay below ~100
+    constexpr int IPT = (NZ >= 2 && 6 * NZ * 2 * sizeof(T) / 4 <= 100) ? 2 : 1;
+    constexpr int THREADS = 32 * ((NZ + IPT - 1) / IPT);
+    auto kern = coupling_batched_kernel<T, NZ, IPT, STAGES>;
     const size_t smem = (size_t)STAGES * 3 * NZ * 32 * sizeof(C);
     static int occ_blocks = 0;
     cudaError_t err;
@@ -230,13 +254,13 @@ static cudaError_t launch_coupling_batched_nz(const void* bank, void* spec, int 
             if (err != cudaSuccess) return err;
         }
         int nb = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, 32 * NZ, smem);
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, THREADS, smem);
         if (err != cudaSuccess) return err;
         occ_blocks = nb < 1 ? 1 : nb;
     }
     long long grid = (long long)num_sms * occ_blocks;
     if (grid > n_tiles) grid = n_tiles;
-    kern<<<(unsigned)grid, 32 * NZ, smem, st>>>((const T*)bank, (C*)spec, batch, n_tiles, ks);
+    kern<<<(unsigned)grid, THREADS, smem, st>>>((const T*)bank, (C*)spec, batch, n_tiles, ks);
     return cudaGetLastError();
 }
 

@@ -209,11 +209,14 @@ struct RowFFT {
         const C* twp;                              // twt + j
         unsigned st[NSTAGES][R];                   // st[s][u]: store base of butterfly u after stage s
         unsigned ld;                               // load base: element j of the row
+        int bar;                                   // named barrier of the row (TPR > 32)
     };
 
-    // the row synchronises among its own threads only: one warp (or less) when TPR <= 32
-    static __device__ __forceinline__ void sync() {
-        if (TPR <= 32) __syncwarp(); else __syncthreads();
+    // the row synchronises among its own threads only: within one warp when TPR <= 32, else on
+    // the row's own named barrier (bar.sync id, TPR), so rows of a CTA never wait for each other
+    static __device__ __forceinline__ void sync(const Ctx& c) {
+        if (TPR <= 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(c.bar), "n"(TPR) : "memory");
     }
 
     template <int LNS, int SIDX>
@@ -231,10 +234,13 @@ struct RowFFT {
         }
     }
 
+    // r: row slot in the CTA (at most 15 slots when TPR > 32: named barriers 1..15);
     // rowaddr: shared-space address of the row's buffer pair (ROW_BYTES aligned); rx < min(16, N)
     // is XOR-ed into every element index of the row (lets a caller read the rows "transposed",
     // lanes along rows, without bank conflicts); twt: per-thread twiddle table.
-    static __device__ __forceinline__ void init(Ctx& c, unsigned rowaddr, int j, int rx, const C* __restrict__ twt) {
+    static __device__ __forceinline__ void init(Ctx& c, int r, unsigned rowaddr, int j, int rx,
+                                                const C* __restrict__ twt) {
+        c.bar = r + 1;
         c.ld = rowaddr ^ ((unsigned)(swz(j) ^ rx) << SH);
         c.twp = twt + j;
         if constexpr (REGTW) {
@@ -284,7 +290,7 @@ struct RowFFT {
 #pragma unroll
                 for (int t = 0; t < RAD; ++t)
                     sts(c.st[SIDX][u] ^ (((unsigned)swz(t * NS) << SH) ^ (PAR ? BUF_BYTES : 0u)), v[u + t * U]);
-            sync();
+            sync(c);
 #pragma unroll
             for (int q = 0; q < R; ++q) v[q] = lds<C>(elem_addr<PAR>(c, q));
             stage<LNS + LR, SIDX + 1, PAR ^ 1>(v, c);
@@ -297,7 +303,7 @@ struct RowFFT {
     // only hazard between consecutive rows is an odd number of exchanges: one more barrier then.
     static __device__ __forceinline__ void run(C (&v)[R], const Ctx& c) {
         stage<0, 0, 0>(v, c);
-        if constexpr (EXCH & 1) sync();
+        if constexpr (EXCH & 1) sync(c);
     }
 };
 

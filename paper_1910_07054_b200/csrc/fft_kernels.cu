@@ -36,6 +36,14 @@ __device__ __forceinline__ unsigned smem_base_aligned(unsigned align) {
     return (smem_u32(smem_raw) + align - 1) & ~(align - 1);
 }
 
+// Element-index XOR of row r in a block of 2^log2rb rows (x kernels).  The transposed phase reads
+// one element index from 2^log2rb rows at a time, lanes along the rows: spreading r over bits
+// 0..3 of the index makes those rows hit different banks (r itself for 16 rows, 2r for 8, ...).
+__device__ __forceinline__ int row_xor(int r, int log2rb, int N) {
+    const int sh = log2rb < 4 ? 4 - log2rb : 0;
+    return (r << sh) & 15 & (N - 1);
+}
+
 // ------------------------------------------------------------------------------------------
 // S1: forward x.  A real row of 2N samples (only the first N non-zero if ZP) is packed as N
 // complex z[t] = x[2t] + i x[2t+1]; Z = DFT_N(z); X[k] = E[k] + W_2N^k O[k] with
@@ -62,8 +70,8 @@ fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb,
     const int rr = tid & (rb - 1), kk = tid >> log2rb;       // phase 2
     const unsigned base = smem_base_aligned(F::ROW_BYTES);
     typename F::Ctx c;
-    F::init(c, base + r * F::ROW_BYTES, j, r & 15 & (N - 1), twt);
-    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)(rr & 15 & (N - 1)) << SH) ^ (PZ ? F::BUF_BYTES : 0u);
+    F::init(c, r, base + r * F::ROW_BYTES, j, row_xor(r, log2rb, N), twt);
+    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)row_xor(rr, log2rb, N) << SH) ^ (PZ ? F::BUF_BYTES : 0u);
 
     long long blk = (long long)blockIdx.x * bpc;
     const int nit = (int)((nblocks - blk < bpc) ? nblocks - blk : bpc);
@@ -140,8 +148,8 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
     const int rr = tid & (rb - 1), kk = tid >> log2rb;       // phase 1
     const unsigned base = smem_base_aligned(F::ROW_BYTES);
     typename F::Ctx c;
-    F::init(c, base + r * F::ROW_BYTES, j, r & 15 & (N - 1), twt);
-    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)(rr & 15 & (N - 1)) << SH) ^ F::BUF_BYTES;
+    F::init(c, r, base + r * F::ROW_BYTES, j, row_xor(r, log2rb, N), twt);
+    const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)row_xor(rr, log2rb, N) << SH) ^ F::BUF_BYTES;
 
     long long blk = (long long)blockIdx.x * bpc;
     const int nit = (int)((nblocks - blk < bpc) ? nblocks - blk : bpc);
@@ -220,7 +228,7 @@ ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long
     const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
     const int rpc = blockDim.x >> F::LOG2TPR;
     typename F::Ctx c;
-    F::init(c, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
+    F::init(c, r, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
 
     const long long g0 = (long long)blockIdx.x * gpc;
     const int nit = (int)((ngroups - g0 < gpc) ? ngroups - g0 : gpc);
@@ -271,7 +279,7 @@ iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long lo
     const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);
     const int rpc = blockDim.x >> F::LOG2TPR;
     typename F::Ctx c;
-    F::init(c, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
+    F::init(c, r, smem_base_aligned(F::ROW_BYTES) + r * F::ROW_BYTES, j, 0, twt);
 
     const long long g0 = (long long)blockIdx.x * gpc;
     const int nit = (int)((ngroups - g0 < gpc) ? ngroups - g0 : gpc);
