@@ -43,14 +43,6 @@ template <> struct BankVec<double, 1> {
     static __device__ __forceinline__ void ld(const double* p, double v[1]) { v[0] = __ldcs(p); }
 };
 
-__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gsrc) {
-    unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;\n" ::"r"(d), "l"(gsrc));
-}
-__device__ __forceinline__ void cp_async_wait_all() {
-    asm volatile("cp.async.commit_group;\ncp.async.wait_group 0;\n" ::: "memory");
-}
-
 template <typename T, int KPT>
 __global__ void __launch_bounds__(512)
 coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
@@ -149,11 +141,6 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
 // memory once for both (ncu: the one-layer version is shared-memory-bandwidth bound).
 // Tile = 32 wavevectors (hfft_api.cu picks tile_k = 32 when this kernel applies).
 // ------------------------------------------------------------------------------------------
-template <int N> __device__ __forceinline__ void cp_async_wait_group() {
-    asm volatile("cp.async.wait_group %0;\n" ::"n"(N) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-
 template <typename T, int NZ, int IPT, int STAGES>
 __global__ void __launch_bounds__(32 * ((NZ + IPT - 1) / IPT))
 coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int batch, long long n_tiles,

@@ -129,9 +129,11 @@ fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb,
 // ------------------------------------------------------------------------------------------
 // S5: inverse x (complex-to-real, crop to the first N reals = first N/2 complex outputs).
 // Z~[k] = E~ + i O~,  E~ = X[k] + conj X[N-k],  O~ = (X[k] - conj X[N-k]) W_2N^{-k};
-// z~ = IDFT_N(Z~) holds x~[2t] + i x~[2t+1].  Same row blocks as S1: phase 1 reads the
-// transposed X^ with lanes along y and writes Z~ to the rows in shared memory, phase 2 is the
-// row transform; only the first half of its outputs is stored (fused crop).
+// z~ = IDFT_N(Z~) holds x~[2t] + i x~[2t+1].  Same row blocks as S1: the block's tile of the
+// transposed X^ ([N + 1][rb]) is brought to shared memory by cp.async ONE BLOCK AHEAD (ncu: without
+// it the kernel waits on the global loads, long_scoreboard 7.2 + barrier 3.6 per issue); phase 1
+// reads it with lanes along y and writes Z~ to the rows, phase 2 is the row transform; only the
+// first half of its outputs is stored (fused crop).
 // ------------------------------------------------------------------------------------------
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(XCfg<T>::MAXT, XCfg<T>::MINB)
@@ -143,13 +145,17 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
     constexpr int IT = R > 1 ? R / 2 : 1;
     constexpr int RS = R > 1 ? R / 2 : 1;                    // stores per thread (crop)
     constexpr int PZ = 1;                                    // Z~ sits in buffer 1: exchange 0 writes buffer 0
-    const int tid = threadIdx.x, rb = 1 << log2rb;
+    const int tid = threadIdx.x, rb = 1 << log2rb, nthreads = blockDim.x;
     const int r = tid >> F::LOG2TPR, j = tid & (TPR - 1);    // phase 2
     const int rr = tid & (rb - 1), kk = tid >> log2rb;       // phase 1
     const unsigned base = smem_base_aligned(F::ROW_BYTES);
     typename F::Ctx c;
     F::init(c, r, base + r * F::ROW_BYTES, j, row_xor(r, log2rb, N), twt);
     const unsigned zrow = (base + rr * F::ROW_BYTES) ^ ((unsigned)row_xor(rr, log2rb, N) << SH) ^ F::BUF_BYTES;
+    // staging tile of the block's X^ values, [N + 1][rb], filled by cp.async one block ahead
+    const unsigned stg = base + rb * F::ROW_BYTES;
+    const int log2cpr = log2rb + SH - 4;                     // 16-byte chunks per kx row of the tile
+    const int nchunks = (N + 1) << log2cpr;
 
     long long blk = (long long)blockIdx.x * bpc;
     const int nit = (int)((nblocks - blk < bpc) ? nblocks - blk : bpc);
@@ -159,27 +165,43 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
     C* zout = reinterpret_cast<C*>(out) + (blk * rb + r) * (N / 2) + j;
     const long long zstep = (long long)rb * (N / 2);
 
+    auto fetch = [&](long long pl, int yy) {
+        const char* src = reinterpret_cast<const char*>(xhat + pl * (long long)(N + 1) * rows_per_plane + yy);
+        for (int x = tid; x < nchunks; x += nthreads) {
+            const int k = x >> log2cpr, ch = x & ((1 << log2cpr) - 1);
+            cp_async16(stg + ((unsigned)x << 4), src + ((long long)k * rows_per_plane * sizeof(C) + ((long long)ch << 4)));
+        }
+        cp_async_commit();
+    };
+    fetch(plane, y0);
+
     for (int it0 = 0; it0 < nit; ++it0) {
-        const C* xp = xhat + plane * (long long)(N + 1) * rows_per_plane + y0 + rr;
+        cp_async_wait_group<0>();
+        __syncthreads();                                     // the tile has landed for every thread
+        const unsigned sx = stg + ((unsigned)rr << SH);
+        const unsigned kstride = (unsigned)rb << SH;
 #pragma unroll
         for (int it = 0; it < IT; ++it) {
             const int k = kk + TPR * it;
             if (it == 0 && kk == 0) {
-                const C x0 = xp[0], xn = xp[(long long)N * rows_per_plane];     // DC and Nyquist (both real)
+                const C x0 = lds<C>(sx), xn = lds<C>(sx + N * kstride);            // DC and Nyquist (both real)
                 const C e = cadd(x0, cconj(xn)), d = csub(x0, cconj(xn));
                 sts(zrow, mk<T>(e.x - d.y, e.y + d.x));
-                const C xm = xp[(long long)(N / 2) * rows_per_plane];
+                const C xm = lds<C>(sx + (N / 2) * kstride);
                 sts(zrow ^ ((unsigned)swz(N / 2) << SH), mk<T>(2 * xm.x, -2 * xm.y));
             } else {
-                const C xk = xp[(long long)k * rows_per_plane];
-                const C xn = cconj(xp[(long long)(N - k) * rows_per_plane]);
+                const C xk = lds<C>(sx + k * kstride);
+                const C xn = cconj(lds<C>(sx + (N - k) * kstride));
                 const C e = cadd(xk, xn);
                 const C o = mul_pi(cmulc(csub(xk, xn), __ldg(tw + k)));        // i O~
                 sts(zrow ^ ((unsigned)swz(k) << SH), cadd(e, o));              // Z~[k] = E~ + i O~
                 sts(zrow ^ ((unsigned)swz(N - k) << SH), cconj(csub(e, o)));   // Z~[N-k] = conj(E~ - i O~)
             }
         }
-        __syncthreads();
+        __syncthreads();                                     // Z~ complete; the staging tile is free
+        y0 += rb;
+        if (y0 == rows_per_plane) { y0 = 0; ++plane; }
+        if (it0 + 1 < nit) fetch(plane, y0);                 // next block's tile flies during the transform
         C v[R];
 #pragma unroll
         for (int q = 0; q < R; ++q) v[q] = lds<C>(F::template elem_addr<PZ>(c, q));
@@ -187,9 +209,6 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
 #pragma unroll
         for (int q = 0; q < RS; ++q) zout[q * TPR] = v[q];
         zout += zstep;
-        __syncthreads();                                     // rows are free for the next block's Z~
-        y0 += rb;
-        if (y0 == rows_per_plane) { y0 = 0; ++plane; }
     }
 }
 
@@ -413,7 +432,7 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
     const int log2rb = x_log2_rows_per_block<T>(log2nx, rows_per_plane), rb = 1 << log2rb;
     const int threads = rb * fft_tpr(log2nx);
     const size_t row_bytes = (size_t)2 * N * sizeof(C);
-    const size_t smem = (rb + 1) * row_bytes;
+    const size_t smem = (rb + 1) * row_bytes + (size_t)(N + 1) * rb * sizeof(C);   // rows + alignment slack + X^ tile
     const long long nblocks = (long long)nplanes * rows_per_plane / rb;
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_X(log2nx, {
