@@ -135,6 +135,36 @@ hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *M
                             void *stream);
 
 /*
+ * Geometry update for layer-thickness optimisation (section 4
+ * "Layer thickness optimization": the thickness of one layer is varied by a
+ * Newton iteration and the tensor is rebuilt each time).
+ * Sets dz[k] = dz_new and rebuilds ONLY the layer pairs whose tensor changes:
+ * N_ij depends on (dz_i, dz_j, zeta_i - zeta_j) alone, so pairs with both layers
+ * below k, or both above k, keep their entries; row i = k is rebuilt for all j,
+ * rows i < k for j >= k, rows i > k for j <= k.  Same arithmetic as
+ * hfft_build_tensor (double-double evaluation, fp64 FFT).  Enqueues on
+ * `stream` and synchronises it before returning (frees its scratch memory).
+ * Errors: EINVAL (k out of range, dz_new not positive / finite), ESTATE (tensor
+ * not built), ENOMEM, ECUDA (the plan then needs hfft_build_tensor again).
+ */
+hfft_status hfft_update_dz(hfft_plan *plan, int k, double dz_new, void *stream);
+
+/*
+ * Fused reductions of the field.  With a non-NULL
+ * `sums_device` (DEVICE pointer to B*3*nz*2 doubles, caller-owned, 8-byte
+ * aligned) every following hfft_demag / hfft_demag_host zeroes that array and
+ * its last kernel (S5) accumulates, for plane p = (b*3 + c)*nz + i,
+ *     sums[2p]   = sum over the nx*ny cells of h_c(., ., i)          (<H_c> of layer i times nx*ny;
+ *                  the quantity the paper's thickness optimisation drives to zero)
+ *     sums[2p+1] = sum over the cells of m_c * h_c, m as passed to the call
+ *                  (demagnetization energy: E = -(mu0/2) dx dy sum_i dz_i Ms_i sum_c sums[2p+1]
+ *                  when Ms was passed per layer; Eq.1-2 define H as the cell average)
+ * in fp64 (floating-point atomics: the summation order is not fixed).
+ * NULL switches the reductions off (the default; no cost).  Errors: EINVAL.
+ */
+hfft_status hfft_plan_set_reduction(hfft_plan *plan, double *sums_device);
+
+/*
  * Per-stage device timing.  With profiling on, hfft_demag brackets every stage
  * with CUDA events on `stream`.  hfft_profile_read synchronises on the last
  * event and returns, for each of the HFFT_NUM_STAGES stages, the SUM of elapsed

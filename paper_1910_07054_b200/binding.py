@@ -24,7 +24,8 @@ MAX_NZ = 256
 
 # every symbol include/hfft.h declares
 EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_info", "hfft_plan_set_buffers",
-           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_profile_enable", "hfft_profile_read",
+           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_update_dz", "hfft_plan_set_reduction",
+           "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
 
 
@@ -64,6 +65,8 @@ def lib():
         L.hfft_build_tensor.argtypes = [vp, vp]
         L.hfft_demag.argtypes = [vp, vp, dp, vp, vp]
         L.hfft_demag_host.argtypes = [vp, vp, dp, vp, vp]
+        L.hfft_update_dz.argtypes = [vp, ctypes.c_int, ctypes.c_double, vp]
+        L.hfft_plan_set_reduction.argtypes = [vp, vp]
         L.hfft_profile_enable.argtypes = [vp, ctypes.c_int]
         L.hfft_profile_read.argtypes = [vp, dp, ip]
         L.hfft_read_bank.argtypes = [vp, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp]
@@ -146,6 +149,15 @@ def demag_host(plan, m_host_ptr, Ms, h_host_ptr, stream=0, nz=None):
                                  ctypes.c_void_p(stream)), plan)
 
 
+def update_dz(plan, k, dz_new, stream=0):
+    _check(lib().hfft_update_dz(plan, int(k), float(dz_new), ctypes.c_void_p(stream)), plan)
+
+
+def plan_set_reduction(plan, sums_ptr):
+    """sums_ptr: device address of B*3*nz*2 doubles, or 0 / None to switch the reductions off."""
+    _check(lib().hfft_plan_set_reduction(plan, ctypes.c_void_p(sums_ptr or None)), plan)
+
+
 def profile_enable(plan, on=True):
     _check(lib().hfft_profile_enable(plan, 1 if on else 0), plan)
 
@@ -219,6 +231,17 @@ class Plan:
             h_host = t.empty_like(m_host).pin_memory()
         demag_host(self.handle, m_host.data_ptr(), Ms, h_host.data_ptr(), self._stream(), nz=self.nz)
         return h_host
+
+    def update_dz(self, k, dz_new):
+        update_dz(self.handle, k, dz_new, self._stream())
+
+    def set_reduction(self, on=True):
+        """Returns the device tensor [B][3][nz][2] = (sum of h_c, sum of m_c h_c) per plane that every
+        following demag call fills (None when switched off)."""
+        t = self.torch
+        self.sums = t.zeros((self.batch, 3, self.nz, 2), dtype=t.float64, device="cuda") if on else None
+        plan_set_reduction(self.handle, self.sums.data_ptr() if on else 0)
+        return self.sums
 
     def close(self):
         if self.handle:

@@ -135,10 +135,14 @@ fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb,
 // reads it with lanes along y and writes Z~ to the rows, phase 2 is the row transform; only the
 // first half of its outputs is stored (fused crop).
 // ------------------------------------------------------------------------------------------
-template <typename T, int LOG2N>
+// RED (hfft_plan_set_reduction): the epilogue also accumulates, per plane, the sum of h
+// and the sum of m h over the plane's cells (doubles, one atomicAdd per warp and block) into
+// sums[plane][2] -- the layer average <H_z> of PAPER.md:209 and the m.H sums of the demagnetization energy.
+template <typename T, int LOG2N, bool RED>
 __global__ void __launch_bounds__(XCfg<T>::MAXT, XCfg<T>::MINB)
 ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, int rows_per_plane,
-             const HFFT_C* __restrict__ tw, const HFFT_C* __restrict__ twt, long long nblocks, int bpc) {
+             const HFFT_C* __restrict__ tw, const HFFT_C* __restrict__ twt, long long nblocks, int bpc,
+             const T* __restrict__ m, double* __restrict__ sums) {
     typedef HFFT_C C;
     typedef RowFFT<T, LOG2N, true, false, false> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR, SH = F::SH;
@@ -163,6 +167,7 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
     long long plane = blk / bpp;
     int y0 = (int)(blk - plane * bpp) << log2rb;
     C* zout = reinterpret_cast<C*>(out) + (blk * rb + r) * (N / 2) + j;
+    const C* zm = reinterpret_cast<const C*>(m) + (blk * rb + r) * (N / 2) + j;
     const long long zstep = (long long)rb * (N / 2);
 
     auto fetch = [&](long long pl, int yy) {
@@ -199,6 +204,7 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
             }
         }
         __syncthreads();                                     // Z~ complete; the staging tile is free
+        const long long cur_plane = plane;
         y0 += rb;
         if (y0 == rows_per_plane) { y0 = 0; ++plane; }
         if (it0 + 1 < nit) fetch(plane, y0);                 // next block's tile flies during the transform
@@ -208,6 +214,27 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
         F::run(v, c);
 #pragma unroll
         for (int q = 0; q < RS; ++q) zout[q * TPR] = v[q];
+        if constexpr (RED) {
+            double sh = 0.0, smh = 0.0;
+#pragma unroll
+            for (int q = 0; q < RS; ++q) {
+                const C mm = zm[q * TPR];
+                sh += (double)v[q].x + (double)v[q].y;
+                smh += (double)v[q].x * (double)mm.x + (double)v[q].y * (double)mm.y;
+            }
+            if (nthreads >= 32) {                            // a block lies in one plane: so does the warp
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) {
+                    sh += __shfl_xor_sync(0xffffffffu, sh, o);
+                    smh += __shfl_xor_sync(0xffffffffu, smh, o);
+                }
+            }
+            if (nthreads < 32 || (tid & 31) == 0) {
+                atomicAdd(sums + 2 * cur_plane, sh);
+                atomicAdd(sums + 2 * cur_plane + 1, smh);
+            }
+            zm += zstep;
+        }
         zout += zstep;
     }
 }
@@ -426,7 +453,7 @@ cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, in
 
 template <typename T>
 cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw,
-                         const void* twt, int num_sms, cudaStream_t st) {
+                         const void* twt, int num_sms, const T* m, double* sums, cudaStream_t st) {
     typedef HFFT_C C;
     const int N = 1 << log2nx;
     const int log2rb = x_log2_rows_per_block<T>(log2nx, rows_per_plane), rb = 1 << log2rb;
@@ -435,15 +462,30 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
     const size_t smem = (rb + 1) * row_bytes + (size_t)(N + 1) * rb * sizeof(C);   // rows + alignment slack + X^ tile
     const long long nblocks = (long long)nplanes * rows_per_plane / rb;
     cudaError_t err = cudaErrorInvalidValue;
+    if (sums) {
+        HFFT_DISPATCH_X(log2nx, {
+            auto kern = ifftx_kernel<T, L, true>;
+            static LaunchCache lc;
+            int occ = 1;
+            if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+                unsigned grid; int bpc;
+                chunk_grid(nblocks, num_sms, occ, grid, bpc);
+                kern<<<grid, threads, smem, st>>>((const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
+                                                  (const C*)twt, nblocks, bpc, m, sums);
+                err = cudaGetLastError();
+            }
+        })
+        return err;
+    }
     HFFT_DISPATCH_X(log2nx, {
-        auto kern = ifftx_kernel<T, L>;
+        auto kern = ifftx_kernel<T, L, false>;
         static LaunchCache lc;
         int occ = 1;
         if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int bpc;
             chunk_grid(nblocks, num_sms, occ, grid, bpc);
             kern<<<grid, threads, smem, st>>>((const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
-                                              (const C*)twt, nblocks, bpc);
+                                              (const C*)twt, nblocks, bpc, m, sums);
             err = cudaGetLastError();
         }
     })
@@ -510,8 +552,8 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
 template cudaError_t launch_fftx_fwd<float, true>(const float*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
 template cudaError_t launch_fftx_fwd<double, true>(const double*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
 template cudaError_t launch_fftx_fwd<double, false>(const double*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
-template cudaError_t launch_ifftx<float>(const void*, float*, int, int, int, const void*, const void*, int, cudaStream_t);
-template cudaError_t launch_ifftx<double>(const void*, double*, int, int, int, const void*, const void*, int, cudaStream_t);
+template cudaError_t launch_ifftx<float>(const void*, float*, int, int, int, const void*, const void*, int, const float*, double*, cudaStream_t);
+template cudaError_t launch_ifftx<double>(const void*, double*, int, int, int, const void*, const void*, int, const double*, double*, cudaStream_t);
 template cudaError_t launch_ffty_fwd<float, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
 template cudaError_t launch_ffty_fwd<double, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
 template cudaError_t launch_ffty_fwd<double, false>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);

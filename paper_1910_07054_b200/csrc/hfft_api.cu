@@ -31,6 +31,7 @@ struct hfft_plan {
     // length-2ny row transforms (fft.cuh).  *64: fp64 copies for the setup (aliases for an fp64 plan).
     void *tw_x = nullptr, *twt_x = nullptr, *twt_y = nullptr;
     void *tw_x64 = nullptr, *twt_x64 = nullptr, *twt_y64 = nullptr;
+    double* sums = nullptr;                          // hfft_plan_set_reduction: [B][3][nz][2] on device
     bool profiling = false;
     int prof_calls = 0;
     std::vector<cudaEvent_t> prof_events;            // (HFFT_NUM_STAGES + 1) per call
@@ -265,7 +266,7 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     if ((e = cudaMalloc(&scratch, sb)) != cudaSuccess)
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
     std::string msg;
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, st, msg);
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, -1, st, msg);
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
     if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_build_tensor: " + msg);
@@ -297,7 +298,10 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
                                        p->num_sms, st)))
     STAGE(2, (launch_coupling<T>(p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded, p->num_sms, st)))
     STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y, p->num_sms, st)))
-    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, st)))
+    if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
+        return fail_cuda(p, "cudaMemsetAsync(sums)", e);
+    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, (const T*)m,
+                              p->sums, st)))
 #undef STAGE
     if (ev) {
         if ((e = cudaEventRecord(ev[HFFT_NUM_STAGES], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);
@@ -316,6 +320,36 @@ hfft_status hfft_demag(hfft_plan* plan, const void* m, const double* Ms, void* h
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag: call hfft_build_tensor first");
     cudaStream_t st = (cudaStream_t)stream;
     return plan->prec == HFFT_F32 ? demag_impl<float>(plan, m, Ms, h, st) : demag_impl<double>(plan, m, Ms, h, st);
+}
+
+hfft_status hfft_plan_set_reduction(hfft_plan* plan, double* sums_device) {
+    if (!plan) return HFFT_EINVAL;
+    if (((size_t)sums_device & 7)) return fail(plan, HFFT_EINVAL, "hfft_plan_set_reduction: sums must be 8-byte aligned");
+    plan->sums = sums_device;
+    return HFFT_OK;
+}
+
+hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (k < 0 || k >= plan->nz) return fail(plan, HFFT_EINVAL, "hfft_update_dz: layer index out of range");
+    if (!(dz_new > 0) || !isfinite(dz_new)) return fail(plan, HFFT_EINVAL, "hfft_update_dz: dz must be positive and finite");
+    if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_update_dz: call hfft_build_tensor first");
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    plan->dz[k] = dz_new;
+    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
+                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
+    void* scratch = nullptr;
+    if ((e = cudaMalloc(&scratch, build_scratch_bytes(g))) != cudaSuccess)
+        return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
+    std::string msg;
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, k, st, msg);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    cudaFree(scratch);
+    if (e != cudaSuccess) { plan->built = false; return fail(plan, HFFT_ECUDA, "hfft_update_dz: " + msg); }
+    if (e2 != cudaSuccess) { plan->built = false; return fail_cuda(plan, "hfft_update_dz: cudaStreamSynchronize", e2); }
+    return HFFT_OK;
 }
 
 hfft_status hfft_demag_host(hfft_plan* plan, const void* m_host, const double* Ms, void* h_host, void* stream) {

@@ -21,9 +21,10 @@ template <typename T, bool ZP>
 cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, int rows_per_plane, int nz,
                             const double* ms_host, const void* tw2nx, const void* twt_nx, int num_sms,
                             cudaStream_t st);
+// sums != nullptr: also accumulate sums[plane][2] += (sum of out, sum of m * out) over the plane's cells
 template <typename T>
 cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw2nx,
-                         const void* twt_nx, int num_sms, cudaStream_t st);
+                         const void* twt_nx, int num_sms, const T* m, double* sums, cudaStream_t st);
 // forward y: X^ rows [nplanes * (nx+1)][N/2 if ZP else N] -> k side [nplanes][ks], k = kx * N + ky;
 // nz_rot > 0 multiplies the z-component planes by i
 template <typename T, bool ZP>
@@ -54,8 +55,9 @@ struct BuildGeom {
 };
 size_t build_scratch_bytes(const BuildGeom& g);
 // fills `bank` (plan precision); fp64 tables on device: tw2nx (2nx entries) and the per-thread
-// tables of the length-nx and length-2ny row transforms
+// tables of the length-nx and length-2ny row transforms.  changed < 0: every layer pair; else only
+// the pairs whose tensor depends on the thickness of layer `changed` (hfft_update_dz)
 cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx_f64, const void* twt_nx_f64,
-                       const void* twt_2ny_f64, cudaStream_t st, std::string& err);
+                       const void* twt_2ny_f64, int changed, cudaStream_t st, std::string& err);
 
 }  // namespace hfft

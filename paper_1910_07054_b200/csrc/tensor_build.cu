@@ -31,11 +31,11 @@ __constant__ int kParZ[6] = {+1, +1, +1, +1, -1, -1};
 
 // phi[b][c][Q][P], Q in [0, ny], P in [0, nx], z = zeta[a] - zeta[b]
 __global__ void __launch_bounds__(128)
-lattice_kernel(double2* __restrict__ phi, const double2* __restrict__ zeta, int a, int nx, int ny, int nz,
+lattice_kernel(double2* __restrict__ phi, const double2* __restrict__ zeta, int a, int b0, int nx, int ny, int nz,
                double dx, double dy) {
     const int P = blockIdx.x * blockDim.x + threadIdx.x;
     const int Q = blockIdx.y;
-    const int b = blockIdx.z;
+    const int b = b0 + blockIdx.z;
     if (P > nx) return;
     dd za = dd_make(zeta[a].x, zeta[a].y), zb = dd_make(zeta[b].x, zeta[b].y);
     dd z = dd_sub(za, zb);
@@ -55,10 +55,10 @@ lattice_kernel(double2* __restrict__ phi, const double2* __restrict__ zeta, int 
 
 // psi[b][c][q][p] = second difference in x and in y of phi, p in [0, nx), q in [0, ny)
 __global__ void __launch_bounds__(128)
-stencil_kernel(double2* __restrict__ psi, const double2* __restrict__ phi, int nx, int ny) {
+stencil_kernel(double2* __restrict__ psi, const double2* __restrict__ phi, int bc0, int nx, int ny) {
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     const int q = blockIdx.y;
-    const int bc = blockIdx.z;          // b * 6 + c
+    const int bc = bc0 + blockIdx.z;    // b * 6 + c
     if (p >= nx) return;
     const int c = bc % 6;
     const double2* f = phi + (size_t)bc * (ny + 1) * (nx + 1);
@@ -170,8 +170,17 @@ size_t build_scratch_bytes(const BuildGeom& g) { return scratch_layout(g).total;
         }                                                                              \
     } while (0)
 
+// Source layers j whose pair (i, j) changes when the thickness of layer `changed` changes (NEXT-1,
+// PAPER.md:205-211): N_ij depends on (dz_i, dz_j, zeta_i - zeta_j) only, so pairs on one side of the
+// changed layer keep their tensor; changed < 0: every pair.
+static void changed_range(int nz, int changed, int i, int& jlo, int& jhi) {
+    jlo = 0; jhi = nz - 1;
+    if (changed < 0 || i == changed) return;
+    if (i < changed) jlo = changed; else jhi = changed;
+}
+
 cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx, const void* twt_nx,
-                       const void* twt_2ny, cudaStream_t st, std::string& err) {
+                       const void* twt_2ny, int changed, cudaStream_t st, std::string& err) {
     const ScratchLayout L = scratch_layout(g);
     unsigned char* base = static_cast<unsigned char*>(scratch);
     double2* d_zeta = reinterpret_cast<double2*>(base + L.zeta);
@@ -198,20 +207,32 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
     const dd inv4pi = dd_make(DD_INV_4PI_HI, DD_INV_4PI_LO);
     for (int a = 0; a <= nz; ++a) {
         {
-            dim3 grid((nx + 1 + 127) / 128, ny + 1, nz + 1);
-            lattice_kernel<<<grid, 128, 0, st>>>(d_phi, d_zeta, a, nx, ny, nz, g.dx, g.dy);
+            // interface a serves target rows a - 1 (upper face) and a (lower face): source interfaces b
+            // in the union of their ranges [jlo, jhi + 1]
+            int blo = nz + 1, bhi = -1;
+            for (int i = a - 1; i <= a; ++i) {
+                if (i < 0 || i >= nz) continue;
+                int jlo, jhi;
+                changed_range(nz, changed, i, jlo, jhi);
+                if (jlo < blo) blo = jlo;
+                if (jhi + 1 > bhi) bhi = jhi + 1;
+            }
+            dim3 grid((nx + 1 + 127) / 128, ny + 1, bhi - blo + 1);
+            lattice_kernel<<<grid, 128, 0, st>>>(d_phi, d_zeta, a, blo, nx, ny, nz, g.dx, g.dy);
             HFFT_CK(cudaGetLastError());
-            dim3 grid2((nx + 127) / 128, ny, (nz + 1) * 6);
-            stencil_kernel<<<grid2, 128, 0, st>>>(d_psi[a & 1], d_phi, nx, ny);
+            dim3 grid2((nx + 127) / 128, ny, (bhi - blo + 1) * 6);
+            stencil_kernel<<<grid2, 128, 0, st>>>(d_psi[a & 1], d_phi, blo * 6, nx, ny);
             HFFT_CK(cudaGetLastError());
         }
         if (a == 0) continue;
         const int i = a - 1;
+        int jlo, jhi;
+        changed_range(nz, changed, i, jlo, jhi);
         // -1 / (4 pi dx dy dz_i) in double-double
         dd tau = dd_mul_d(two_prod(g.dx, g.dy), g.dz[i]);
         dd coef = dd_neg(dd_div(inv4pi, tau));
-        for (int j0 = 0; j0 < nz; j0 += L.jc) {
-            const int jn = (nz - j0 < L.jc) ? nz - j0 : L.jc;
+        for (int j0 = jlo; j0 <= jhi; j0 += L.jc) {
+            const int jn = (jhi + 1 - j0 < L.jc) ? jhi + 1 - j0 : L.jc;
             dim3 grid((nx + 127) / 128, ny, jn * 6);
             assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
                                                   make_double2(coef.hi, coef.lo));
