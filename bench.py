@@ -63,12 +63,13 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def algorithmic_bytes(w):
-    """what the shipped storage must move per hfft_demag call."""
+def algorithmic_bytes(w, n_slots=None):
+    """what the shipped storage must move per hfft_demag call.
+    n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank)."""
     s = 4 if w.precision == "f32" else 8
     n_k = 2 * w.ny * (w.nx + 1)
     planes = 3 * w.nz * w.B
-    bank = 6 * w.nz * w.nz * n_k * s
+    bank = 6 * (n_slots if n_slots else w.nz * w.nz) * n_k * s
     spec = planes * n_k * 2 * s            # M^ (= H^)
     xhat = planes * w.ny * (w.nx + 1) * 2 * s
     field = planes * w.ny * w.nx * s
@@ -234,7 +235,8 @@ def main():
     h_host = torch.empty_like(m_host).pin_memory()
     Ms = w.Ms
     nbytes = m.numel() * m.element_size()
-    ab = algorithmic_bytes(w)
+    dedup = int(plan.info.dedup)
+    ab = algorithmic_bytes(w, plan.info.n_classes if dedup else None)
     # inputs larger than L2?  otherwise flush L2 between steps (and say so)
     flush = None
     if ab["whole"] < 512 << 20:
@@ -338,6 +340,21 @@ def main():
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
             "setup_s": setup_s,
         }
+        if dedup >= 2:
+            # deduplicated bank held in shared memory: the coupling is bound by the FP32/FP64 FMA pipe, not by HBM
+            # (18 nz^2 n_k B real FMAs; peak = SMs x 128 (fp32) or 64 (fp64) FMA lanes x 2 x clock)
+            flops = 2.0 * 18 * w.nz * w.nz * (2 * w.ny * (w.nx + 1)) * w.B
+            lanes = 128 if w.precision == "f32" else 64
+            alu_peak = 148 * lanes * 2 * clocks["sm_max_mhz"] * 1e6 / 1e12
+            tf = flops / (coup_ms * 1e-3) / 1e12 if coup_ms > 0 else None
+            line["roofline"] = {"bound": "alu", "kernel": "coupling_class_kernel (S3, deduplicated bank)",
+                                "achieved": tf, "peak": alu_peak,
+                                "peak_source": "derived: 148 SMs x %d FMA lanes x 2 flop x sm_max_mhz (DESIGN.md)" % lanes,
+                                "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
+                                "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
+                                "hbm_gbs": achieved, "traffic": None}
+        line["config"]["bank"] = {"dedup": dedup, "slots_per_k": int(plan.info.n_classes if dedup else w.nz * w.nz),
+                                  "bytes": int(plan.info.bank_bytes)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line))

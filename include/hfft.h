@@ -60,11 +60,14 @@ typedef struct {
     int tile_k;               /* wavevectors per bank tile */
     long long n_k;            /* wavevectors in the Hermitian half spectrum: (nx+1) * 2ny */
     long long n_k_padded;     /* n_k rounded up to a multiple of tile_k */
-    size_t bank_bytes;        /* spectral tensor bank: 6 * nz^2 * n_k_padded * sizeof(element) */
+    size_t bank_bytes;        /* spectral tensor bank: 6 * (nz^2 or n_classes) * n_k_padded * sizeof(element) */
     size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging */
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
     int launches_per_demag;   /* kernels hfft_demag enqueues per call */
     int built;                /* 1 once hfft_build_tensor has completed */
+    int n_classes;            /* distinct tensors among the nz^2 layer pairs (hfft_plan_set_dedup) */
+    int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
+                                 shared memory; 3: as 2 with Toeplitz classes (equal thicknesses) */
 } hfft_info;
 
 /*
@@ -85,7 +88,23 @@ hfft_status hfft_plan_create(hfft_plan **out, int nx, int ny, int nz,
  * hfft_plan_set_buffers.  Errors: EINVAL (B < 1), ESTATE. */
 hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
 
-/* Sizes the plan needs; valid after create / set_batch.  Errors: EINVAL. */
+/*
+ * Bank deduplication.  N_ij depends on (dz_i, dz_j, zeta_i - zeta_j)
+ * alone (Eq.19 with Eq.5/11), so layer pairs that agree in the three
+ * share one tensor ("class"): equal thicknesses -- the equidistant case the paper
+ * compares against, PAPER.md:182-189 -- give 2nz-1 classes instead of nz^2, periodic
+ * multilayers a few per period.  The bank then holds one slot per class
+ * (info.bank_bytes shrinks by nz^2 / n_classes) and, where a k-tile of it fits in
+ * shared memory, the coupling stage stops being HBM-bound (coupling.cu).
+ *   mode 0: off (one slot per pair; required for hfft_update_dz)
+ *   mode 1: automatic (default): on when n_classes <= nz^2 / 2
+ *   mode 2: on
+ * Results are those of the plain bank up to summation order.  Must be called
+ * before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
+ */
+hfft_status hfft_plan_set_dedup(hfft_plan *plan, int mode);
+
+/* Sizes the plan needs; valid after create / set_batch / set_dedup.  Errors: EINVAL. */
 hfft_status hfft_plan_info(const hfft_plan *plan, hfft_info *info);
 
 /*
@@ -145,7 +164,8 @@ hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *M
  * hfft_build_tensor (double-double evaluation, fp64 FFT).  Enqueues on
  * `stream` and synchronises it before returning (frees its scratch memory).
  * Errors: EINVAL (k out of range, dz_new not positive / finite), ESTATE (tensor
- * not built), ENOMEM, ECUDA (the plan then needs hfft_build_tensor again).
+ * not built), EUNSUPPORTED (deduplicated bank: use hfft_plan_set_dedup(plan, 0)),
+ * ENOMEM, ECUDA (the plan then needs hfft_build_tensor again).
  */
 hfft_status hfft_update_dz(hfft_plan *plan, int k, double dz_new, void *stream);
 

@@ -23,7 +23,7 @@ STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
 
 # every symbol include/hfft.h declares
-EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_info", "hfft_plan_set_buffers",
+EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_info", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
@@ -35,7 +35,8 @@ class Info(ctypes.Structure):
                 ("n_k", ctypes.c_longlong), ("n_k_padded", ctypes.c_longlong),
                 ("bank_bytes", ctypes.c_size_t), ("workspace_bytes", ctypes.c_size_t),
                 ("setup_scratch_bytes", ctypes.c_size_t),
-                ("launches_per_demag", ctypes.c_int), ("built", ctypes.c_int)]
+                ("launches_per_demag", ctypes.c_int), ("built", ctypes.c_int),
+                ("n_classes", ctypes.c_int), ("dedup", ctypes.c_int)]
 
 
 class HfftError(RuntimeError):
@@ -60,6 +61,7 @@ def lib():
         L.hfft_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                        ctypes.c_double, ctypes.c_double, dp, ctypes.c_int]
         L.hfft_plan_set_batch.argtypes = [vp, ctypes.c_int]
+        L.hfft_plan_set_dedup.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.hfft_plan_set_buffers.argtypes = [vp, vp, vp]
         L.hfft_build_tensor.argtypes = [vp, vp]
@@ -110,6 +112,11 @@ def plan_create(nx, ny, nz, dx, dy, dz, precision):
 
 def plan_set_batch(plan, batch):
     _check(lib().hfft_plan_set_batch(plan, int(batch)), plan)
+
+
+def plan_set_dedup(plan, mode):
+    """0 off, 1 automatic (default), 2 on."""
+    _check(lib().hfft_plan_set_dedup(plan, int(mode)), plan)
 
 
 def plan_info(plan) -> Info:
@@ -185,7 +192,7 @@ def destroy(plan):
 class Plan:
     """Convenience owner: plan + torch-allocated bank / workspace on the current CUDA device."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True):
+    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -197,6 +204,8 @@ class Plan:
         self.nx, self.ny, self.nz, self.batch = nx, ny, nz, batch
         if batch != 1:
             plan_set_batch(self.handle, batch)
+        if dedup is not None:
+            plan_set_dedup(self.handle, dedup)
         self.info = plan_info(self.handle)
         self._bank = self._ws = None
         if torch_buffers:

@@ -23,30 +23,35 @@
 
 namespace hfft {
 
+// one lane's KPT consecutive bank values: streamed (evict-first: every value is used once) or, for
+// the deduplicated bank, through the read-only cached path (the tile is re-read by every target layer)
+template <bool CACHED, typename V> __device__ __forceinline__ V bank_ld(const V* p) {
+    return CACHED ? __ldg(p) : __ldcs(p);
+}
 template <typename T, int KPT> struct BankVec;
 template <> struct BankVec<float, 4> {
-    static __device__ __forceinline__ void ld(const float* p, float v[4]) {
-        float4 t = __ldcs(reinterpret_cast<const float4*>(p));
+    template <bool CACHED> static __device__ __forceinline__ void ld(const float* p, float v[4]) {
+        float4 t = bank_ld<CACHED>(reinterpret_cast<const float4*>(p));
         v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
     }
 };
 template <> struct BankVec<float, 1> {
-    static __device__ __forceinline__ void ld(const float* p, float v[1]) { v[0] = __ldcs(p); }
+    template <bool CACHED> static __device__ __forceinline__ void ld(const float* p, float v[1]) { v[0] = bank_ld<CACHED>(p); }
 };
 template <> struct BankVec<double, 2> {
-    static __device__ __forceinline__ void ld(const double* p, double v[2]) {
-        double2 t = __ldcs(reinterpret_cast<const double2*>(p));
+    template <bool CACHED> static __device__ __forceinline__ void ld(const double* p, double v[2]) {
+        double2 t = bank_ld<CACHED>(reinterpret_cast<const double2*>(p));
         v[0] = t.x; v[1] = t.y;
     }
 };
 template <> struct BankVec<double, 1> {
-    static __device__ __forceinline__ void ld(const double* p, double v[1]) { v[0] = __ldcs(p); }
+    template <bool CACHED> static __device__ __forceinline__ void ld(const double* p, double v[1]) { v[0] = bank_ld<CACHED>(p); }
 };
 
-template <typename T, int KPT>
+template <typename T, int KPT, bool CLS>
 __global__ void __launch_bounds__(512)
 coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
-                long long ks) {
+                long long ks, int ncls, const unsigned short* __restrict__ cls) {
     typedef HFFT_C C;
     constexpr int TK = 32 * KPT;
     constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk (2 or 1)
@@ -76,12 +81,16 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
             C hx[KPT], hy[KPT], hz[KPT];
 #pragma unroll
             for (int e = 0; e < KPT; ++e) hx[e] = hy[e] = hz[e] = mk<T>((T)0, (T)0);
-            const T* bt = bank + ((tile * nz + i) * nz) * (6LL * TK) + lane * KPT;
+            // deduplicated bank (CLS): the slot of pair (i, j) is its tensor class; the tile is then small
+            // and re-read by every target layer, so it is served from L1 / L2
+            const T* bt = CLS ? bank + tile * ncls * (6LL * TK) + lane * KPT
+                              : bank + ((tile * nz + i) * nz) * (6LL * TK) + lane * KPT;
 #pragma unroll 2
             for (int j = 0; j < nz; ++j) {
                 T a[6][KPT];
+                const int slot = CLS ? (int)cls[i * nz + j] : j;
 #pragma unroll
-                for (int c = 0; c < 6; ++c) BankVec<T, KPT>::ld(bt + (j * 6 + c) * TK, a[c]);
+                for (int c = 0; c < 6; ++c) BankVec<T, KPT>::template ld<CLS>(bt + (slot * 6 + c) * TK, a[c]);
                 C m[3][KPT];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -217,6 +226,171 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
     }
 }
 
+// ------------------------------------------------------------------------------------------
+// Deduplicated bank: layer pairs with identical (dz_i, dz_j, zeta_i - zeta_j) share
+// one tensor class, bank layout [tile][class][6][32].  With few classes (equal thicknesses: 2 nz - 1
+// instead of nz^2, the configuration of the paper's equidistant comparison) the
+// bank of a k-tile fits in shared memory next to M^, HBM traffic drops by nz / 2, and the stage is
+// bound by the FMA pipe and the shared-memory bandwidth instead.
+//
+// A lane owns one wavevector, a warp IPT CONSECUTIVE target layers i0 .. i0 + IPT - 1.  Per source
+// layer j a thread reads M^_j(k) once (3 complex) for its IPT targets.
+//  - generic classes: 6 bank reals per (i, j) from shared memory (class index from a shared table);
+//  - TOEP (class = i - j + nz - 1): the tensors of (i0 + p, j), p < IPT, are a sliding window over
+//    the class index; going from j to j + 1 the window moves by one, so ONE class (6 reals) is
+//    loaded per j and the other IPT - 1 stay in registers (the j loop is unrolled by IPT so that
+//    the window rotates by register renaming).  Shared-memory wavefronts per j: 6 + 6 for
+//    9 IPT packed FMAs -- FMA-bound at IPT = 8.
+// H^ is written straight to global memory (in place of M^, whose tile was read completely first).
+// ------------------------------------------------------------------------------------------
+// threads per CTA = 32 * ceil(nz / IPT), nz <= kClassMaxNz
+constexpr int kClassMaxNz = 96;
+// (fp32: shared memory limits nz to 96; fp64: to 47, and its registers count double)
+template <typename T, int IPT> struct ClassCfg {
+    static constexpr int W = IPT * (int)sizeof(T) / 4;    // register weight of the per-thread state
+    static constexpr int MAXT = W >= 8 ? 384 : (W == 4 ? 768 : 512);
+};
+
+template <typename T, int IPT, bool TOEP>
+__global__ void __launch_bounds__(ClassCfg<T, IPT>::MAXT, 1)
+coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, const unsigned short* __restrict__ cls,
+                      int nz, int ncls, int batch, long long n_tiles, long long ks) {
+    typedef HFFT_C C;
+    constexpr int TK = 32;
+    constexpr int CHUNK_C = 16 / sizeof(C), CPP = TK / CHUNK_C;
+    constexpr int CHUNK_T = 16 / sizeof(T);
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    T* sb = reinterpret_cast<T*>(smem_raw);                                        // [ncls][6][32]
+    C* sm = reinterpret_cast<C*>(smem_raw + (size_t)ncls * 6 * TK * sizeof(T));    // [3 nz][32]
+    unsigned short* scls = reinterpret_cast<unsigned short*>(sm + 3 * nz * TK);    // [nz][nz] (generic)
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int np = 3 * nz;
+    const int i0 = warp * IPT;
+
+    if (!TOEP) {
+        for (int x = tid; x < nz * nz; x += blockDim.x) scls[x] = cls[x];
+    }
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+        {
+            const T* src = bank + tile * ncls * (6LL * TK);
+            for (int x = tid; x < ncls * 6 * TK / CHUNK_T; x += blockDim.x)
+                cp_async16(sb + x * CHUNK_T, src + x * CHUNK_T);
+        }
+        for (int b = 0; b < batch; ++b) {
+            C* sp = spec + (long long)b * np * ks + tile * TK;
+            for (int x = tid; x < np * CPP; x += blockDim.x) {
+                const int lp = x / CPP, ch = x - lp * CPP;
+                cp_async16(sm + lp * TK + ch * CHUNK_C, sp + (long long)lp * ks + ch * CHUNK_C);
+            }
+            cp_async_wait_all();
+            __syncthreads();
+
+            C hx[IPT], hy[IPT], hz[IPT];
+#pragma unroll
+            for (int p = 0; p < IPT; ++p) hx[p] = hy[p] = hz[p] = mk<T>((T)0, (T)0);
+            T win[IPT][6];
+            if (TOEP) {
+#pragma unroll
+                for (int p = 0; p < IPT; ++p) {
+                    int c0 = i0 + p + nz - 1;                  // class of (i0 + p, j = 0)
+                    if (c0 > ncls - 1) c0 = ncls - 1;          // layers past nz - 1 of the last warp (unused)
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) win[p][c] = sb[(c0 * 6 + c) * TK + lane];
+                }
+            }
+            for (int j0 = 0; j0 < nz; j0 += IPT) {
+#pragma unroll
+                for (int jj = 0; jj < IPT; ++jj) {
+                    const int j = j0 + jj;
+                    if (j < nz) {
+                        const C mx = sm[(0 * nz + j) * TK + lane], my = sm[(1 * nz + j) * TK + lane],
+                                mz = sm[(2 * nz + j) * TK + lane];
+#pragma unroll
+                        for (int p = 0; p < IPT; ++p) {
+                            T a[6];
+                            if (TOEP) {
+#pragma unroll
+                                for (int c = 0; c < 6; ++c) a[c] = win[(p - jj + IPT) % IPT][c];
+                            } else {
+                                int i = i0 + p;
+                                if (i > nz - 1) i = nz - 1;
+                                const int cl = scls[i * nz + j];
+#pragma unroll
+                                for (int c = 0; c < 6; ++c) a[c] = sb[(cl * 6 + c) * TK + lane];
+                            }
+                            hx[p] = caxpy(a[0], mx, hx[p]); hx[p] = caxpy(a[3], my, hx[p]); hx[p] = caxpy(a[4], mz, hx[p]);
+                            hy[p] = caxpy(a[3], mx, hy[p]); hy[p] = caxpy(a[1], my, hy[p]); hy[p] = caxpy(a[5], mz, hy[p]);
+                            hz[p] = caxpy(a[2], mz, hz[p]); hz[p] = caxpy(-a[4], mx, hz[p]); hz[p] = caxpy(-a[5], my, hz[p]);
+                        }
+                        if (TOEP && j + 1 < nz) {
+                            // window for j + 1: targets move up one slot, the freed slot takes (i0, j + 1)
+                            const int cn = i0 - j - 1 + nz - 1;
+#pragma unroll
+                            for (int c = 0; c < 6; ++c) win[(IPT - 1 - jj) % IPT][c] = sb[(cn * 6 + c) * TK + lane];
+                        }
+                    }
+                }
+            }
+#pragma unroll
+            for (int p = 0; p < IPT; ++p) {
+                const int i = i0 + p;
+                if (i < nz) {
+                    sp[(long long)(0 * nz + i) * ks + lane] = hx[p];
+                    sp[(long long)(1 * nz + i) * ks + lane] = hy[p];
+                    sp[(long long)(2 * nz + i) * ks + lane] = hz[p];
+                }
+            }
+            __syncthreads();   // every warp is done with M^ (and, after the last state, the bank) in shared memory
+        }
+    }
+}
+
+size_t coupling_class_smem_bytes(int nz, int n_classes, bool toeplitz, size_t elem) {
+    if (nz > kClassMaxNz) return (size_t)1 << 30;
+    return (size_t)n_classes * 6 * 32 * elem + (size_t)3 * nz * 32 * 2 * elem +
+           (toeplitz ? 0 : (size_t)nz * nz * sizeof(unsigned short));
+}
+
+template <typename T, int IPT, bool TOEP>
+static cudaError_t launch_coupling_class_t(const CouplingArgs& a, cudaStream_t st) {
+    typedef HFFT_C C;
+    auto kern = coupling_class_kernel<T, IPT, TOEP>;
+    const size_t smem = coupling_class_smem_bytes(a.nz, a.n_classes, TOEP, sizeof(T));
+    const int threads = 32 * ((a.nz + IPT - 1) / IPT);
+    if (threads > ClassCfg<T, IPT>::MAXT) return cudaErrorInvalidConfiguration;
+    static size_t smem_done = 0;
+    cudaError_t err;
+    if (smem > 48 * 1024 && smem > smem_done) {
+        err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        smem_done = smem;
+    }
+    int nb = 0;
+    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
+    if (err != cudaSuccess) return err;
+    if (nb < 1) return cudaErrorInvalidConfiguration;
+    long long grid = (long long)a.num_sms * nb;
+    if (grid > a.n_tiles) grid = a.n_tiles;
+    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.cls, a.nz, a.n_classes, a.batch,
+                                                a.n_tiles, a.ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+static cudaError_t launch_coupling_class(const CouplingArgs& a, cudaStream_t st) {
+    // IPT target layers per warp: 8 keeps the Toeplitz window FMA-bound; fewer for thin stacks so that
+    // a CTA still has several warps
+    constexpr int H = sizeof(T) == 4 ? 1 : 2;             // fp64: half the layers per thread
+    if (a.toeplitz) {
+        if (a.nz >= 32 / H) return launch_coupling_class_t<T, 8 / H, true>(a, st);
+        if (a.nz >= 8) return launch_coupling_class_t<T, 4 / H, true>(a, st);
+        return launch_coupling_class_t<T, 1, true>(a, st);
+    }
+    if (a.nz >= 16) return launch_coupling_class_t<T, 4 / H, false>(a, st);
+    if (a.nz >= 8) return launch_coupling_class_t<T, 2 / H, false>(a, st);
+    return launch_coupling_class_t<T, 1, false>(a, st);
+}
+
 // the batched kernel keeps 6 nz reals of the bank per thread: at most 96 32-bit registers
 bool coupling_batched_applies(int nz, int batch, size_t elem) {
     return batch > 1 && (size_t)6 * nz * elem <= 96 * 4;
@@ -273,13 +447,12 @@ static cudaError_t launch_coupling_batched(const void* bank, void* spec, int nz,
 
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem) { return (size_t)3 * nz * tile_k * 2 * elem; }
 
-template <typename T, int KPT>
-static cudaError_t launch_coupling_k(const void* bank, void* spec, int nz, int batch, long long n_tiles, long long ks,
-                                     int num_sms, cudaStream_t st) {
+template <typename T, int KPT, bool CLS>
+static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     typedef HFFT_C C;
-    auto kern = coupling_kernel<T, KPT>;
-    const size_t smem = coupling_smem_bytes(nz, 32 * KPT, sizeof(T));
-    const int warps = nz < 16 ? nz : 16;
+    auto kern = coupling_kernel<T, KPT, CLS>;
+    const size_t smem = coupling_smem_bytes(a.nz, 32 * KPT, sizeof(T));
+    const int warps = a.nz < 16 ? a.nz : 16;
     const int threads = warps * 32;
     static size_t smem_done = 0;
     static int occ_threads = 0, occ_blocks = 0;
@@ -296,25 +469,31 @@ static cudaError_t launch_coupling_k(const void* bank, void* spec, int nz, int b
         if (err != cudaSuccess) return err;
         occ_threads = threads; occ_smem = smem; occ_blocks = nb < 1 ? 1 : nb;
     }
-    long long items = n_tiles * batch;
-    long long grid = (long long)num_sms * occ_blocks;
+    long long items = a.n_tiles * a.batch;
+    long long grid = (long long)a.num_sms * occ_blocks;
     if (grid > items) grid = items;
-    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)bank, (C*)spec, nz, batch, n_tiles, ks);
+    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.nz, a.batch, a.n_tiles, a.ks,
+                                                a.n_classes, a.cls);
     return cudaGetLastError();
 }
 
 template <typename T>
-cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
-                            long long ks, int num_sms, cudaStream_t st) {
+cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
     constexpr int KV = 16 / sizeof(T);
-    if (tile_k == 32 && coupling_batched_applies(nz, batch, sizeof(T)))
-        return launch_coupling_batched<T>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
-    if (tile_k == 32 * KV) return launch_coupling_k<T, KV>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
-    if (tile_k == 32) return launch_coupling_k<T, 1>(bank, spec, nz, batch, n_tiles, ks, num_sms, st);
+    if (a.cls) {
+        if (a.class_kernel) return a.tile_k == 32 ? launch_coupling_class<T>(a, st) : cudaErrorInvalidValue;
+        if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, true>(a, st);
+        if (a.tile_k == 32) return launch_coupling_k<T, 1, true>(a, st);
+        return cudaErrorInvalidValue;
+    }
+    if (a.tile_k == 32 && coupling_batched_applies(a.nz, a.batch, sizeof(T)))
+        return launch_coupling_batched<T>(a.bank, a.spec, a.nz, a.batch, a.n_tiles, a.ks, a.num_sms, st);
+    if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, false>(a, st);
+    if (a.tile_k == 32) return launch_coupling_k<T, 1, false>(a, st);
     return cudaErrorInvalidValue;
 }
 
-template cudaError_t launch_coupling<float>(const void*, void*, int, int, int, long long, long long, int, cudaStream_t);
-template cudaError_t launch_coupling<double>(const void*, void*, int, int, int, long long, long long, int, cudaStream_t);
+template cudaError_t launch_coupling<float>(const CouplingArgs&, cudaStream_t);
+template cudaError_t launch_coupling<double>(const CouplingArgs&, cudaStream_t);
 
 }  // namespace hfft

@@ -32,6 +32,12 @@ struct hfft_plan {
     void *tw_x = nullptr, *twt_x = nullptr, *twt_y = nullptr;
     void *tw_x64 = nullptr, *twt_x64 = nullptr, *twt_y64 = nullptr;
     double* sums = nullptr;                          // hfft_plan_set_reduction: [B][3][nz][2] on device
+    // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
+    int dedup_mode = 1;                              // 0 off, 1 auto, 2 on
+    bool dedup = false, toeplitz = false, class_kernel = false;
+    int n_classes = 0;                               // distinct tensors among the nz^2 pairs
+    std::vector<int> pair_class, class_rep;
+    unsigned short* d_cls = nullptr;                 // device copy of pair_class (dedup only)
     bool profiling = false;
     int prof_calls = 0;
     std::vector<cudaEvent_t> prof_events;            // (HFFT_NUM_STAGES + 1) per call
@@ -127,18 +133,29 @@ static cudaError_t upload_thread_twiddles(int log2N, bool f32, void** out) {
     return upload_complex(re, im, f32, out);
 }
 
+static BuildGeom make_geom(const hfft_plan* p) {
+    BuildGeom g{p->nx, p->ny, p->nz, p->log2nx, p->log2ny, p->dx, p->dy, p->dz.data(),
+                p->tile_k, p->n_k, p->n_k_padded, p->prec, p->num_sms};
+    if (p->dedup) { g.pair_class = p->pair_class.data(); g.class_rep = p->class_rep.data(); g.n_classes = p->n_classes; }
+    return g;
+}
+
 static void plan_sizes(hfft_plan* p) {
     const size_t e = p->elem;
     p->n_k = 2LL * p->ny * (p->nx + 1);
+    // deduplicated bank: automatically once at most half of the pairs carry a tensor of their own
+    p->dedup = p->dedup_mode == 2 || (p->dedup_mode == 1 && 2 * p->n_classes <= p->nz * p->nz);
+    p->class_kernel = p->dedup && coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
     // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
     const int wide = 32 * (int)(16 / e);
     p->tile_k = (p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148)) ? wide : 32;
     while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
     if (p->tile_k != wide) p->tile_k = 32;
-    if (coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
+    if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
+    if (p->class_kernel) p->tile_k = 32;
     p->n_tiles = (p->n_k + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
-    p->bank_bytes = (size_t)6 * p->nz * p->nz * (size_t)p->n_k_padded * e;
+    p->bank_bytes = (size_t)6 * (p->dedup ? p->n_classes : p->nz * p->nz) * (size_t)p->n_k_padded * e;
     const size_t planes = (size_t)3 * p->nz * p->batch;
     auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
     size_t o = 0;
@@ -188,6 +205,8 @@ hfft_status hfft_plan_create(hfft_plan** out, int nx, int ny, int nz, double dx,
     p->dz.assign(dz, dz + nz);
     p->device = dev; p->num_sms = prop.multiProcessorCount;
     p->elem = precision == HFFT_F32 ? 4 : 8;
+    pair_classes(nz, p->dz.data(), p->pair_class, p->class_rep, p->toeplitz);
+    p->n_classes = (int)p->class_rep.size();
     plan_sizes(p);
     if (coupling_smem_bytes(nz, p->tile_k, p->elem) > 200 * 1024) {
         delete p;
@@ -206,17 +225,27 @@ hfft_status hfft_plan_set_batch(hfft_plan* plan, int batch) {
     return HFFT_OK;
 }
 
+hfft_status hfft_plan_set_dedup(hfft_plan* plan, int mode) {
+    if (!plan) return HFFT_EINVAL;
+    if (mode < 0 || mode > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_dedup: mode must be 0, 1 or 2");
+    if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_dedup: after build / set_buffers");
+    plan->dedup_mode = mode;
+    plan_sizes(plan);
+    return HFFT_OK;
+}
+
 hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     if (!plan || !info) return HFFT_EINVAL;
     info->nx = plan->nx; info->ny = plan->ny; info->nz = plan->nz; info->batch = plan->batch;
     info->precision = plan->prec; info->tile_k = plan->tile_k;
     info->n_k = plan->n_k; info->n_k_padded = plan->n_k_padded;
     info->bank_bytes = plan->bank_bytes; info->workspace_bytes = plan->ws_bytes;
-    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
-                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
+    BuildGeom g = make_geom(plan);
     info->setup_scratch_bytes = build_scratch_bytes(g);
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
+    info->n_classes = plan->n_classes;
+    info->dedup = plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0;
     return HFFT_OK;
 }
 
@@ -259,8 +288,14 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
             plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
         }
     }
-    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
-                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
+    if (plan->dedup && !plan->d_cls) {
+        std::vector<unsigned short> c16(plan->pair_class.begin(), plan->pair_class.end());
+        if ((e = cudaMalloc(&plan->d_cls, c16.size() * sizeof(unsigned short))) != cudaSuccess)
+            return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(class table): ") + cudaGetErrorString(e));
+        if ((e = cudaMemcpy(plan->d_cls, c16.data(), c16.size() * sizeof(unsigned short), cudaMemcpyHostToDevice)) != cudaSuccess)
+            return fail_cuda(plan, "cudaMemcpy(class table)", e);
+    }
+    BuildGeom g = make_geom(plan);
     void* scratch = nullptr;
     const size_t sb = build_scratch_bytes(g);
     if ((e = cudaMalloc(&scratch, sb)) != cudaSuccess)
@@ -296,7 +331,10 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
                                        p->num_sms, st)))
     STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y,
                                        p->num_sms, st)))
-    STAGE(2, (launch_coupling<T>(p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded, p->num_sms, st)))
+    const CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
+                          p->dedup ? p->n_classes : p->nz * p->nz, p->dedup ? p->d_cls : nullptr,
+                          p->class_kernel, p->toeplitz, p->num_sms};
+    STAGE(2, (launch_coupling<T>(ca, st)))
     STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y, p->num_sms, st)))
     if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
         return fail_cuda(p, "cudaMemsetAsync(sums)", e);
@@ -334,12 +372,13 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
     if (k < 0 || k >= plan->nz) return fail(plan, HFFT_EINVAL, "hfft_update_dz: layer index out of range");
     if (!(dz_new > 0) || !isfinite(dz_new)) return fail(plan, HFFT_EINVAL, "hfft_update_dz: dz must be positive and finite");
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_update_dz: call hfft_build_tensor first");
+    if (plan->dedup)
+        return fail(plan, HFFT_EUNSUPPORTED, "hfft_update_dz: the bank is deduplicated; create the plan with hfft_plan_set_dedup(plan, 0)");
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
     if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
     plan->dz[k] = dz_new;
-    BuildGeom g{plan->nx, plan->ny, plan->nz, plan->log2nx, plan->log2ny, plan->dx, plan->dy, plan->dz.data(),
-                plan->tile_k, plan->n_k, plan->n_k_padded, plan->prec, plan->num_sms};
+    BuildGeom g = make_geom(plan);
     void* scratch = nullptr;
     if ((e = cudaMalloc(&scratch, build_scratch_bytes(g))) != cudaSuccess)
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
@@ -413,7 +452,9 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     const double unscale = -4.0 * p->nx * p->ny;
     std::vector<unsigned char> buf((size_t)tk * p->elem);
     for (long long t = 0; t < p->n_tiles; ++t) {
-        const size_t off = ((((size_t)t * p->nz + i) * p->nz + j) * 6 + c) * tk * p->elem;
+        const size_t ncls = p->dedup ? p->n_classes : (size_t)p->nz * p->nz;
+        const size_t slot = p->dedup ? p->pair_class[(size_t)i * p->nz + j] : (size_t)i * p->nz + j;
+        const size_t off = (((size_t)t * ncls + slot) * 6 + c) * tk * p->elem;
         e = cudaMemcpy(buf.data(), static_cast<unsigned char*>(p->bank) + off, (size_t)tk * p->elem, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, "cudaMemcpy(bank)", e);
         for (int kk = 0; kk < tk; ++kk) {
@@ -432,6 +473,7 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (plan->own_ws && plan->ws) cudaFree(plan->ws);
     if (plan->tw_x != plan->tw_x64) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
     cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
+    if (plan->d_cls) cudaFree(plan->d_cls);
     for (auto& ev : plan->prof_events) cudaEventDestroy(ev);
     delete plan;
     return HFFT_OK;

@@ -35,10 +35,22 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
                          const void* twt_N, int num_sms, cudaStream_t st);
 
 // ---- coupling.cu ----
-// H^ = bank * M^ in place on the k side.  bank layout [tile][i][j][6][tile_k].
+// H^ = bank * M^ in place on the k side.  bank layout [tile][class][6][tile_k]; class = i*nz+j (cls == nullptr)
+// or cls[i*nz+j] (deduplicated bank, device table).
+struct CouplingArgs {
+    const void* bank; void* spec;
+    int nz, batch, tile_k;
+    long long n_tiles, ks;
+    int n_classes;                 // nz*nz without deduplication
+    const unsigned short* cls;     // device, [nz*nz], or nullptr
+    bool class_kernel;             // bank tile in shared memory (coupling_class_applies)
+    bool toeplitz;                 // cls[i*nz+j] == i - j + nz - 1
+    int num_sms;
+};
 template <typename T>
-cudaError_t launch_coupling(const void* bank, void* spec, int nz, int batch, int tile_k, long long n_tiles,
-                            long long ks, int num_sms, cudaStream_t st);
+cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st);
+// shared-memory-resident class kernel: needs tile_k == 32 and this many bytes per CTA
+size_t coupling_class_smem_bytes(int nz, int n_classes, bool toeplitz, size_t elem);
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem);
 // batched register-resident-bank kernel (B > 1, small nz); it needs tile_k == 32
 bool coupling_batched_applies(int nz, int batch, size_t elem);
@@ -52,7 +64,14 @@ struct BuildGeom {
     long long n_k, n_k_padded;
     int prec;              // hfft_precision
     int num_sms;
+    // deduplicated bank: host tables pair -> class [nz*nz], class -> representative pair
+    // i*nz+j [n_classes]; pair_class == nullptr: one slot per pair (class = i*nz+j)
+    const int* pair_class = nullptr;
+    const int* class_rep = nullptr;
+    int n_classes = 0;
 };
+// tensor classes of the layer pairs: pairs with identical (dz_i, dz_j, zeta_i - zeta_j) share one tensor
+void pair_classes(int nz, const double* dz, std::vector<int>& cls, std::vector<int>& rep, bool& toeplitz);
 size_t build_scratch_bytes(const BuildGeom& g);
 // fills `bank` (plan precision); fp64 tables on device: tw2nx (2nx entries) and the per-thread
 // tables of the length-nx and length-2ny row transforms.  changed < 0: every layer pair; else only

@@ -20,6 +20,11 @@
 // zz even in X and Y; xy odd, odd; xz odd, even; yz even, odd); a full (not zero-padded) fp64
 // real-to-complex 2-D FFT follows, and the real part (xx, yy, zz, xy) or imaginary part (xz, yz)
 // times -1/(4 nx ny) is stored in the plan precision at bank[tile][i][j][c][k in tile].
+#include <math.h>
+
+#include <map>
+#include <utility>
+
 #include "hfft_internal.h"
 #include "newell_dd.cuh"
 
@@ -116,8 +121,8 @@ assemble_kernel(double* __restrict__ R, const double2* __restrict__ psi_lo /* a 
 
 template <typename T>
 __global__ void __launch_bounds__(256)
-pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, int j0, int jcount, int tile_k,
-            long long n_k, long long n_k_padded, double scale) {
+pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, int j0, int ncls,
+            const unsigned short* __restrict__ cls, int tile_k, long long n_k, long long n_k_padded, double scale) {
     const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int jc = blockIdx.y;          // jl * 6 + c
     if (k >= n_k_padded) return;
@@ -129,12 +134,12 @@ pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, 
     }
     const long long tile = k / tile_k;
     const int kk = (int)(k - tile * tile_k);
-    bank[(((tile * nz + i) * nz + (j0 + jl)) * 6 + c) * tile_k + kk] = (T)v;
-    (void)jcount;
+    const int pr = i * nz + j0 + jl;                       // bank slot = tensor class of the pair
+    bank[((tile * ncls + (cls ? (int)cls[pr] : pr)) * 6 + c) * tile_k + kk] = (T)v;
 }
 
 struct ScratchLayout {
-    size_t zeta, phi, psi0, psi1, R, X, Y, total;
+    size_t zeta, cls, phi, psi0, psi1, R, X, Y, total;
     int jc;
 };
 
@@ -149,6 +154,7 @@ static ScratchLayout scratch_layout(const BuildGeom& g) {
     L.jc = (int)jc;
     size_t o = 0;
     L.zeta = o; o += al((size_t)(g.nz + 1) * 16);
+    L.cls = o;  o += al((size_t)g.nz * g.nz * sizeof(unsigned short));
     L.phi = o;  o += al((size_t)(g.nz + 1) * 6 * (g.ny + 1) * (g.nx + 1) * 16);
     L.psi0 = o; o += al((size_t)(g.nz + 1) * 6 * nxy * 16);
     L.psi1 = o; o += al((size_t)(g.nz + 1) * 6 * nxy * 16);
@@ -170,13 +176,69 @@ size_t build_scratch_bytes(const BuildGeom& g) { return scratch_layout(g).total;
         }                                                                              \
     } while (0)
 
-// Source layers j whose pair (i, j) changes when the thickness of layer `changed` changes (NEXT-1,
-// PAPER.md:205-211): N_ij depends on (dz_i, dz_j, zeta_i - zeta_j) only, so pairs on one side of the
-// changed layer keep their tensor; changed < 0: every pair.
-static void changed_range(int nz, int changed, int i, int& jlo, int& jhi) {
-    jlo = 0; jhi = nz - 1;
-    if (changed < 0 || i == changed) return;
-    if (i < changed) jlo = changed; else jhi = changed;
+// Source layers j of target row i whose tensor has to be evaluated, as inclusive runs [j0, j1].
+//  - hfft_update_dz (changed >= 0): N_ij depends on (dz_i, dz_j, zeta_i - zeta_j) only, so pairs
+//    on one side of the changed layer keep their tensor;
+//  - deduplicated bank (g.pair_class): only the representative pair of every tensor class.
+static std::vector<std::pair<int, int>> row_runs(const BuildGeom& g, int changed, int i) {
+    const int nz = g.nz;
+    std::vector<std::pair<int, int>> runs;
+    if (!g.pair_class) {
+        int jlo = 0, jhi = nz - 1;
+        if (changed >= 0 && i != changed) { if (i < changed) jlo = changed; else jhi = changed; }
+        runs.push_back({jlo, jhi});
+        return runs;
+    }
+    for (int j = 0; j < nz; ++j) {
+        if (g.class_rep[g.pair_class[i * nz + j]] != i * nz + j) continue;
+        if (!runs.empty() && runs.back().second == j - 1) runs.back().second = j;
+        else runs.push_back({j, j});
+    }
+    return runs;
+}
+
+// Tensor classes: N_ij is a function of (dz_i, dz_j, Z_ij = zeta_i - zeta_j) alone (PAPER.md:150
+// Eq.19 with Eq.5/11), so pairs that agree in all three share one bank slot.  dz must agree bit for bit, Z (a
+// double-double difference of the interface coordinates) to 2^-80 of the stack height.  If the class depends on
+// i - j only (equal thicknesses: the z-convolution of Eq.24 is a Toeplitz one, the case of the paper's equidistant
+// comparison) the classes are numbered i - j + nz - 1.
+void pair_classes(int nz, const double* dz, std::vector<int>& cls, std::vector<int>& rep, bool& toeplitz) {
+    std::vector<dd> zeta(nz + 1);
+    zeta[0] = dd_make(0.0, 0.0);
+    for (int k = 0; k < nz; ++k) zeta[k + 1] = dd_add_d(zeta[k], dz[k]);
+    const double tol = ldexp(zeta[nz].hi, -80);
+    struct Key {
+        double a, b, z;
+        bool operator<(const Key& o) const { return a != o.a ? a < o.a : (b != o.b ? b < o.b : z < o.z); }
+    };
+    std::map<Key, std::vector<int>> seen;        // key -> classes with that (dz_i, dz_j, Z.hi)
+    std::vector<dd> zcls;
+    cls.assign((size_t)nz * nz, 0);
+    rep.clear();
+    for (int i = 0; i < nz; ++i)
+        for (int j = 0; j < nz; ++j) {
+            const dd Z = dd_sub(zeta[i], zeta[j]);
+            std::vector<int>& cand = seen[Key{dz[i], dz[j], Z.hi}];
+            int c = -1;
+            for (int t : cand) {
+                const dd d = dd_sub(Z, zcls[t]);
+                if (fabs(d.hi) <= tol) { c = t; break; }
+            }
+            if (c < 0) { c = (int)rep.size(); rep.push_back(i * nz + j); zcls.push_back(Z); cand.push_back(c); }
+            cls[(size_t)i * nz + j] = c;
+        }
+    toeplitz = nz > 1;
+    for (int i = 0; i + 1 < nz && toeplitz; ++i)
+        for (int j = 0; j + 1 < nz; ++j)
+            if (cls[(size_t)i * nz + j] != cls[(size_t)(i + 1) * nz + j + 1]) { toeplitz = false; break; }
+    if (toeplitz && (int)rep.size() == 2 * nz - 1) {
+        rep.assign(2 * nz - 1, 0);
+        for (int i = 0; i < nz; ++i)
+            for (int j = 0; j < nz; ++j) cls[(size_t)i * nz + j] = i - j + nz - 1;
+        for (int d = -(nz - 1); d <= nz - 1; ++d) rep[d + nz - 1] = d >= 0 ? d * nz : -d;
+    } else {
+        toeplitz = false;
+    }
 }
 
 cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void* tw2nx, const void* twt_nx,
@@ -200,56 +262,65 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
         zeta[k + 1] = make_double2(acc.hi, acc.lo);
     }
     HFFT_CK(cudaMemcpyAsync(d_zeta, zeta.data(), sizeof(double2) * (nz + 1), cudaMemcpyHostToDevice, st));
-    HFFT_CK(cudaStreamSynchronize(st));   // `zeta` is pageable host memory
+    unsigned short* d_cls = nullptr;
+    std::vector<unsigned short> cls16;
+    if (g.pair_class) {
+        d_cls = reinterpret_cast<unsigned short*>(base + L.cls);
+        cls16.assign(g.pair_class, g.pair_class + (size_t)nz * nz);
+        HFFT_CK(cudaMemcpyAsync(d_cls, cls16.data(), cls16.size() * sizeof(unsigned short), cudaMemcpyHostToDevice, st));
+    }
+    const int ncls = g.pair_class ? g.n_classes : nz * nz;
+    HFFT_CK(cudaStreamSynchronize(st));   // `zeta`, `cls16` are pageable host memory
     HFFT_CK(cudaMemsetAsync(d_R, 0, (size_t)L.jc * 6 * 4 * nx * ny * 8, st));   // slots p = nx, q = ny stay 0
 
     const double scale = -1.0 / (4.0 * (double)nx * (double)ny);
     const dd inv4pi = dd_make(DD_INV_4PI_HI, DD_INV_4PI_LO);
+    std::vector<std::vector<std::pair<int, int>>> runs(nz);
+    for (int i = 0; i < nz; ++i) runs[i] = row_runs(g, changed, i);
     for (int a = 0; a <= nz; ++a) {
         {
             // interface a serves target rows a - 1 (upper face) and a (lower face): source interfaces b
             // in the union of their ranges [jlo, jhi + 1]
             int blo = nz + 1, bhi = -1;
             for (int i = a - 1; i <= a; ++i) {
-                if (i < 0 || i >= nz) continue;
-                int jlo, jhi;
-                changed_range(nz, changed, i, jlo, jhi);
-                if (jlo < blo) blo = jlo;
-                if (jhi + 1 > bhi) bhi = jhi + 1;
+                if (i < 0 || i >= nz || runs[i].empty()) continue;
+                if (runs[i].front().first < blo) blo = runs[i].front().first;
+                if (runs[i].back().second + 1 > bhi) bhi = runs[i].back().second + 1;
             }
-            dim3 grid((nx + 1 + 127) / 128, ny + 1, bhi - blo + 1);
-            lattice_kernel<<<grid, 128, 0, st>>>(d_phi, d_zeta, a, blo, nx, ny, nz, g.dx, g.dy);
-            HFFT_CK(cudaGetLastError());
-            dim3 grid2((nx + 127) / 128, ny, (bhi - blo + 1) * 6);
-            stencil_kernel<<<grid2, 128, 0, st>>>(d_psi[a & 1], d_phi, blo * 6, nx, ny);
-            HFFT_CK(cudaGetLastError());
+            if (bhi >= blo) {
+                dim3 grid((nx + 1 + 127) / 128, ny + 1, bhi - blo + 1);
+                lattice_kernel<<<grid, 128, 0, st>>>(d_phi, d_zeta, a, blo, nx, ny, nz, g.dx, g.dy);
+                HFFT_CK(cudaGetLastError());
+                dim3 grid2((nx + 127) / 128, ny, (bhi - blo + 1) * 6);
+                stencil_kernel<<<grid2, 128, 0, st>>>(d_psi[a & 1], d_phi, blo * 6, nx, ny);
+                HFFT_CK(cudaGetLastError());
+            }
         }
         if (a == 0) continue;
         const int i = a - 1;
-        int jlo, jhi;
-        changed_range(nz, changed, i, jlo, jhi);
         // -1 / (4 pi dx dy dz_i) in double-double
         dd tau = dd_mul_d(two_prod(g.dx, g.dy), g.dz[i]);
         dd coef = dd_neg(dd_div(inv4pi, tau));
-        for (int j0 = jlo; j0 <= jhi; j0 += L.jc) {
-            const int jn = (jhi + 1 - j0 < L.jc) ? jhi + 1 - j0 : L.jc;
-            dim3 grid((nx + 127) / 128, ny, jn * 6);
-            assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
-                                                  make_double2(coef.hi, coef.lo));
-            HFFT_CK(cudaGetLastError());
-            HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, g.log2nx, jn * 6, 2 * ny, 0, nullptr, tw2nx, twt_nx,
-                                                    g.num_sms, st)));
-            HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, twt_2ny, g.num_sms,
-                                                    st)));
-            dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
-            if (g.prec == HFFT_F32)
-                pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, jn, g.tile_k, g.n_k,
-                                                          g.n_k_padded, scale);
-            else
-                pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, jn, g.tile_k, g.n_k,
-                                                           g.n_k_padded, scale);
-            HFFT_CK(cudaGetLastError());
-        }
+        for (const auto& run : runs[i])
+            for (int j0 = run.first; j0 <= run.second; j0 += L.jc) {
+                const int jn = (run.second + 1 - j0 < L.jc) ? run.second + 1 - j0 : L.jc;
+                dim3 grid((nx + 127) / 128, ny, jn * 6);
+                assemble_kernel<<<grid, 128, 0, st>>>(d_R, d_psi[i & 1], d_psi[a & 1], nx, ny, j0,
+                                                      make_double2(coef.hi, coef.lo));
+                HFFT_CK(cudaGetLastError());
+                HFFT_CK((launch_fftx_fwd<double, false>(d_R, d_X, g.log2nx, jn * 6, 2 * ny, 0, nullptr, tw2nx, twt_nx,
+                                                        g.num_sms, st)));
+                HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, twt_2ny,
+                                                        g.num_sms, st)));
+                dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
+                if (g.prec == HFFT_F32)
+                    pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, ncls, d_cls, g.tile_k, g.n_k,
+                                                              g.n_k_padded, scale);
+                else
+                    pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, ncls, d_cls, g.tile_k,
+                                                               g.n_k, g.n_k_padded, scale);
+                HFFT_CK(cudaGetLastError());
+            }
     }
     HFFT_CK(cudaStreamSynchronize(st));
     return cudaSuccess;

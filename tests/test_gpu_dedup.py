@@ -1,0 +1,159 @@
+"""SURVEY 8f-2 on the GPU: deduplicated tensor bank (hfft_plan_set_dedup) -- tensor classes, the
+shared-memory class kernel (generic and Toeplitz window) and the class-indexed streaming kernel,
+all against the CPU oracle through the C ABI.  -m gpu.
+"""
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1910_07054_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL = {"f32": 2e-6, "f64": 1e-12}
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    from paper_1910_07054_b200 import binding
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    binding.lib()
+    return binding
+
+
+def _relerr(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+def _field(hb, w, m, dedup, batch=1):
+    import torch
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=batch, dedup=dedup)
+    plan.build_tensor()
+    dt = torch.float32 if w.precision == "f32" else torch.float64
+    H = plan.demag(torch.from_numpy(m).to(dt).cuda(), w.Ms).double().cpu().numpy()
+    return plan, H
+
+
+def _expected_classes(dz):
+    """Distinct (dz_i, dz_j, zeta_i - zeta_j) in exact rational arithmetic (Eq.19)."""
+    fz = [Fraction(float(v)) for v in dz]
+    zeta = [sum(fz[:k], Fraction(0)) for k in range(len(dz))]
+    return len({(fz[i], fz[j], zeta[i] - zeta[j]) for i in range(len(dz)) for j in range(len(dz))})
+
+
+# dz exactly representable so that "equal Z" is an exact statement
+STACKS = {
+    "equal5": [1.0] * 5,
+    "equal8": [0.75] * 8,
+    "equal12": [1.5] * 12,
+    "equal33": [0.5] * 33,                       # Toeplitz window, ragged last warp (33 = 4*8 + 1)
+    "period2x4": [1.0, 0.5] * 4,                 # [A/B]x4 multilayer: generic classes
+    "period3x6": [1.0, 0.25, 2.0] * 6,           # 18 layers: generic classes, 4 targets per warp
+    "saf": [5.0, 1.0, 5.0, 1.0, 3.0],            # one coincidence only: automatic mode leaves it off
+}
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("stack", list(STACKS))
+def test_dedup_field_matches_oracle(hb, stack, prec):
+    dz = np.array(STACKS[stack])
+    nz = len(dz)
+    w = W.small(16, 8, nz, precision=prec, seed=31 + nz, dz=dz)
+    m = w.m_rounded()
+    plan, H = _field(hb, w, m, dedup=2)
+    info = hb.plan_info(plan.handle)
+    assert info.n_classes == _expected_classes(dz)
+    if stack.startswith("equal"):
+        assert info.n_classes == 2 * nz - 1 and info.dedup == 3
+    else:
+        assert info.dedup == 2
+    assert info.bank_bytes == 6 * info.n_classes * info.n_k_padded * (4 if prec == "f32" else 8)
+    ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    # automatic mode: on iff at most half of the pairs carry their own tensor
+    auto = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, dz, prec)
+    assert (hb.plan_info(auto.handle).dedup != 0) == (2 * info.n_classes <= nz * nz)
+    auto.close()
+    plan.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_dedup_bank_equals_plain_bank(hb, prec):
+    """Every pair reads, through its class, the tensor it would have had in the plain bank."""
+    dz = np.array([1.0, 0.5, 1.0, 0.5, 1.0, 2.0])
+    w = W.small(8, 16, 6, precision=prec, seed=9, dz=dz)
+    a = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, dz, prec, dedup=0)
+    b = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, dz, prec, dedup=2)
+    a.build_tensor()
+    b.build_tensor()
+    assert hb.plan_info(b.handle).n_classes == _expected_classes(dz) < 36
+    for i in range(6):
+        for j in range(6):
+            for c in range(6):
+                x, y = hb.read_bank(a.handle, i, j, c), hb.read_bank(b.handle, i, j, c)
+                assert np.abs(x - y).max() <= 1e-13 * max(np.abs(x).max(), 1e-30)
+    a.close()
+    b.close()
+
+
+def test_dedup_on_a_stack_without_duplicates(hb):
+    """mode 2 with nz^2 classes: same field as the plain bank (generic class kernel, no savings)."""
+    w = W.small(32, 16, 9, precision="f32", seed=4)
+    m = w.m_rounded()
+    p0, H0 = _field(hb, w, m, dedup=0)
+    p2, H2 = _field(hb, w, m, dedup=2)
+    assert hb.plan_info(p2.handle).n_classes == 81 and hb.plan_info(p2.handle).dedup == 2
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H0, ref) <= TOL["f32"] and _relerr(H2, ref) <= TOL["f32"]
+    assert _relerr(H2, H0) <= 1e-6
+    p0.close()
+    p2.close()
+
+
+@pytest.mark.parametrize("prec,nz", [("f64", 50), ("f32", 100)])
+def test_dedup_streaming_kernel_when_the_tile_does_not_fit(hb, prec, nz):
+    """Equal thicknesses with too many layers for the shared-memory kernel: class-indexed streaming kernel."""
+    dz = np.full(nz, 0.5)
+    w = W.small(8, 8, nz, precision=prec, seed=nz, dz=dz)
+    m = w.m_rounded()
+    plan, H = _field(hb, w, m, dedup=1)
+    info = hb.plan_info(plan.handle)
+    assert info.dedup == 1 and info.n_classes == 2 * nz - 1
+    ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    plan.close()
+
+
+@pytest.mark.parametrize("stack", ["equal12", "period2x4"])
+def test_dedup_batched(hb, stack):
+    dz = np.array(STACKS[stack])
+    w = W.small(16, 16, len(dz), precision="f32", B=3, seed=21, dz=dz)
+    m = w.m_rounded()
+    plan, H = _field(hb, w, m, dedup=1, batch=3)
+    assert hb.plan_info(plan.handle).dedup >= 2
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f32"]
+    plan.close()
+
+
+def test_dedup_errors(hb):
+    dz = np.ones(6)
+    p = hb.Plan(8, 8, 6, 1.0, 1.0, dz, "f64")
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_set_dedup(p.handle, 3)
+    assert e.value.status == hb.EINVAL
+    with pytest.raises(hb.HfftError) as e:          # buffers already handed over: sizes are fixed
+        hb.plan_set_dedup(p.handle, 0)
+    assert e.value.status == hb.ESTATE
+    p.build_tensor()
+    assert hb.plan_info(p.handle).dedup == 3
+    with pytest.raises(hb.HfftError) as e:
+        p.update_dz(2, 1.5)
+    assert e.value.status == hb.EUNSUPPORTED
+    p.close()
+    q = hb.Plan(8, 8, 6, 1.0, 1.0, dz, "f64", dedup=0)
+    q.build_tensor()
+    q.update_dz(2, 1.5)                              # allowed on the plain bank
+    q.close()
