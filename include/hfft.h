@@ -65,7 +65,8 @@ typedef struct {
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
     int launches_per_demag;   /* kernels hfft_demag enqueues per call */
     int built;                /* 1 once hfft_build_tensor has completed */
-    int n_classes;            /* distinct tensors among the nz^2 layer pairs (hfft_plan_set_dedup) */
+    int n_classes;            /* bank slots a deduplicated bank needs: distinct tensors among the nz^2 layer pairs;
+                                 nz for equal thicknesses (N_ij and N_ji then differ by the sign of xz, yz only) */
     int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
                                  shared memory; 3: as 2 with Toeplitz classes (equal thicknesses) */
 } hfft_info;
@@ -92,7 +93,8 @@ hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
  * Bank deduplication.  N_ij depends on (dz_i, dz_j, zeta_i - zeta_j)
  * alone (Eq.19 with Eq.5/11), so layer pairs that agree in the three
  * share one tensor ("class"): equal thicknesses -- the equidistant case the paper
- * compares against, PAPER.md:182-189 -- give 2nz-1 classes instead of nz^2, periodic
+ * compares against, PAPER.md:182-189 -- give nz classes instead of nz^2 (2nz-1 values
+ * of i-j, folded by reciprocity to |i-j|), periodic
  * multilayers a few per period.  The bank then holds one slot per class
  * (info.bank_bytes shrinks by nz^2 / n_classes) and, where a k-tile of it fits in
  * shared memory, the coupling stage stops being HBM-bound (coupling.cu).

@@ -51,7 +51,7 @@ template <> struct BankVec<double, 1> {
 template <typename T, int KPT, bool CLS>
 __global__ void __launch_bounds__(512)
 coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
-                long long ks, int ncls, const unsigned short* __restrict__ cls) {
+                long long ks, int ncls, const unsigned short* __restrict__ cls, int fold) {
     typedef HFFT_C C;
     constexpr int TK = 32 * KPT;
     constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk (2 or 1)
@@ -91,6 +91,10 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                 const int slot = CLS ? (int)cls[i * nz + j] : j;
 #pragma unroll
                 for (int c = 0; c < 6; ++c) BankVec<T, KPT>::template ld<CLS>(bt + (slot * 6 + c) * TK, a[c]);
+                if (CLS && fold && i < j) {               // folded Toeplitz classes: N_{-d} = N_d with xz, yz negated
+#pragma unroll
+                    for (int e = 0; e < KPT; ++e) { a[4][e] = -a[4][e]; a[5][e] = -a[5][e]; }
+                }
                 C m[3][KPT];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -236,8 +240,9 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
 // A lane owns one wavevector, a warp IPT CONSECUTIVE target layers i0 .. i0 + IPT - 1.  Per source
 // layer j a thread reads M^_j(k) once (3 complex) for its IPT targets.
 //  - generic classes: 6 bank reals per (i, j) from shared memory (class index from a shared table);
-//  - TOEP (class = i - j + nz - 1): the tensors of (i0 + p, j), p < IPT, are a sliding window over
-//    the class index; going from j to j + 1 the window moves by one, so ONE class (6 reals) is
+//  - TOEP (equal thicknesses: the tensor depends on d = i - j only; slot |d|, xz and yz negated for
+//    d < 0, so the tile holds nz classes): the tensors of (i0 + p, j), p < IPT, are a sliding window
+//    over d; going from j to j + 1 the window moves by one, so ONE class (6 reals) is
 //    loaded per j and the other IPT - 1 stay in registers (the j loop is unrolled by IPT so that
 //    the window rotates by register renaming).  Shared-memory wavefronts per j: 6 + 6 for
 //    9 IPT packed FMAs -- FMA-bound at IPT = 8.
@@ -245,14 +250,15 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
 // ------------------------------------------------------------------------------------------
 // threads per CTA = 32 * ceil(nz / IPT), nz <= kClassMaxNz
 constexpr int kClassMaxNz = 96;
-// (fp32: shared memory limits nz to 96; fp64: to 47, and its registers count double)
+// (fp32: nz <= 96; fp64: nz <= 64 and its registers count double)
 template <typename T, int IPT> struct ClassCfg {
     static constexpr int W = IPT * (int)sizeof(T) / 4;    // register weight of the per-thread state
-    static constexpr int MAXT = W >= 8 ? 384 : (W == 4 ? 768 : 512);
+    static constexpr int MAXT = W >= 8 ? (sizeof(T) == 8 ? 512 : 384) : (W == 4 ? 768 : 512);
 };
 
-template <typename T, int IPT, bool TOEP>
-__global__ void __launch_bounds__(ClassCfg<T, IPT>::MAXT, 1)
+// MINB = 2: two CTAs of at most 256 threads per SM (one loads its tiles while the other computes)
+template <typename T, int IPT, bool TOEP, int MINB>
+__global__ void __launch_bounds__(MINB == 2 ? 256 : ClassCfg<T, IPT>::MAXT, MINB)
 coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, const unsigned short* __restrict__ cls,
                       int nz, int ncls, int batch, long long n_tiles, long long ks) {
     typedef HFFT_C C;
@@ -292,7 +298,7 @@ coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, con
             if (TOEP) {
 #pragma unroll
                 for (int p = 0; p < IPT; ++p) {
-                    int c0 = i0 + p + nz - 1;                  // class of (i0 + p, j = 0)
+                    int c0 = i0 + p;                           // d of (i0 + p, j = 0)
                     if (c0 > ncls - 1) c0 = ncls - 1;          // layers past nz - 1 of the last warp (unused)
 #pragma unroll
                     for (int c = 0; c < 6; ++c) win[p][c] = sb[(c0 * 6 + c) * TK + lane];
@@ -324,9 +330,13 @@ coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, con
                         }
                         if (TOEP && j + 1 < nz) {
                             // window for j + 1: targets move up one slot, the freed slot takes (i0, j + 1)
-                            const int cn = i0 - j - 1 + nz - 1;
+                            const int dn = i0 - j - 1;
+                            const int cn = dn < 0 ? -dn : dn;
 #pragma unroll
-                            for (int c = 0; c < 6; ++c) win[(IPT - 1 - jj) % IPT][c] = sb[(cn * 6 + c) * TK + lane];
+                            for (int c = 0; c < 6; ++c) {
+                                const T v = sb[(cn * 6 + c) * TK + lane];
+                                win[(IPT - 1 - jj) % IPT][c] = (c >= 4 && dn < 0) ? -v : v;
+                            }
                         }
                     }
                 }
@@ -346,18 +356,18 @@ coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, con
 }
 
 size_t coupling_class_smem_bytes(int nz, int n_classes, bool toeplitz, size_t elem) {
-    if (nz > kClassMaxNz) return (size_t)1 << 30;
+    if (nz > kClassMaxNz || (elem == 8 && nz > 64)) return (size_t)1 << 30;   // thread limits of ClassCfg
     return (size_t)n_classes * 6 * 32 * elem + (size_t)3 * nz * 32 * 2 * elem +
            (toeplitz ? 0 : (size_t)nz * nz * sizeof(unsigned short));
 }
 
-template <typename T, int IPT, bool TOEP>
+template <typename T, int IPT, bool TOEP, int MINB = 1>
 static cudaError_t launch_coupling_class_t(const CouplingArgs& a, cudaStream_t st) {
     typedef HFFT_C C;
-    auto kern = coupling_class_kernel<T, IPT, TOEP>;
+    auto kern = coupling_class_kernel<T, IPT, TOEP, MINB>;
     const size_t smem = coupling_class_smem_bytes(a.nz, a.n_classes, TOEP, sizeof(T));
     const int threads = 32 * ((a.nz + IPT - 1) / IPT);
-    if (threads > ClassCfg<T, IPT>::MAXT) return cudaErrorInvalidConfiguration;
+    if (threads > (MINB == 2 ? 256 : ClassCfg<T, IPT>::MAXT)) return cudaErrorInvalidConfiguration;
     static size_t smem_done = 0;
     cudaError_t err;
     if (smem > 48 * 1024 && smem > smem_done) {
@@ -382,6 +392,7 @@ static cudaError_t launch_coupling_class(const CouplingArgs& a, cudaStream_t st)
     // a CTA still has several warps
     constexpr int H = sizeof(T) == 4 ? 1 : 2;             // fp64: half the layers per thread
     if (a.toeplitz) {
+        if (a.nz >= 32 / H && a.nz <= 64 / H) return launch_coupling_class_t<T, 8 / H, true, 2>(a, st);
         if (a.nz >= 32 / H) return launch_coupling_class_t<T, 8 / H, true>(a, st);
         if (a.nz >= 8) return launch_coupling_class_t<T, 4 / H, true>(a, st);
         return launch_coupling_class_t<T, 1, true>(a, st);
@@ -473,7 +484,7 @@ static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     long long grid = (long long)a.num_sms * occ_blocks;
     if (grid > items) grid = items;
     kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.nz, a.batch, a.n_tiles, a.ks,
-                                                a.n_classes, a.cls);
+                                                a.n_classes, a.cls, a.toeplitz ? 1 : 0);
     return cudaGetLastError();
 }
 

@@ -449,7 +449,8 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return fail_cuda(p, "cudaDeviceSynchronize", e);
     const int tk = p->tile_k;
-    const double unscale = -4.0 * p->nx * p->ny;
+    // folded Toeplitz classes: the slot holds N_{|i-j|}; xz, yz change sign for i < j
+    const double unscale = -4.0 * p->nx * p->ny * ((p->dedup && p->toeplitz && i < j && c >= 4) ? -1.0 : 1.0);
     std::vector<unsigned char> buf((size_t)tk * p->elem);
     for (long long t = 0; t < p->n_tiles; ++t) {
         const size_t ncls = p->dedup ? p->n_classes : (size_t)p->nz * p->nz;

@@ -201,7 +201,7 @@ static std::vector<std::pair<int, int>> row_runs(const BuildGeom& g, int changed
 // Eq.19 with Eq.5/11), so pairs that agree in all three share one bank slot.  dz must agree bit for bit, Z (a
 // double-double difference of the interface coordinates) to 2^-80 of the stack height.  If the class depends on
 // i - j only (equal thicknesses: the z-convolution of Eq.24 is a Toeplitz one, the case of the paper's equidistant
-// comparison) the classes are numbered i - j + nz - 1.
+// comparison) the classes are folded to |i - j| (see below).
 void pair_classes(int nz, const double* dz, std::vector<int>& cls, std::vector<int>& rep, bool& toeplitz) {
     std::vector<dd> zeta(nz + 1);
     zeta[0] = dd_make(0.0, 0.0);
@@ -232,10 +232,14 @@ void pair_classes(int nz, const double* dz, std::vector<int>& cls, std::vector<i
         for (int j = 0; j + 1 < nz; ++j)
             if (cls[(size_t)i * nz + j] != cls[(size_t)(i + 1) * nz + j + 1]) { toeplitz = false; break; }
     if (toeplitz && (int)rep.size() == 2 * nz - 1) {
-        rep.assign(2 * nz - 1, 0);
+        // equal thicknesses: N_ij depends on d = i - j only, and N_{-d} = N_d except that xz and yz change sign
+        // (reciprocity dz_i N_ij(X,Y) = dz_j N_ji(-X,-Y) with the in-plane parities of the components: xx, yy, zz,
+        // xy are even under (X,Y) -> (-X,-Y), xz and yz odd).  One slot per |d|, representative pair (d, 0); the
+        // kernels negate the xz, yz entries for i < j.
+        rep.assign(nz, 0);
         for (int i = 0; i < nz; ++i)
-            for (int j = 0; j < nz; ++j) cls[(size_t)i * nz + j] = i - j + nz - 1;
-        for (int d = -(nz - 1); d <= nz - 1; ++d) rep[d + nz - 1] = d >= 0 ? d * nz : -d;
+            for (int j = 0; j < nz; ++j) cls[(size_t)i * nz + j] = i >= j ? i - j : j - i;
+        for (int d = 0; d < nz; ++d) rep[d] = d * nz;
     } else {
         toeplitz = false;
     }

@@ -49,6 +49,7 @@ STACKS = {
     "equal8": [0.75] * 8,
     "equal12": [1.5] * 12,
     "equal33": [0.5] * 33,                       # Toeplitz window, ragged last warp (33 = 4*8 + 1)
+    "equal70": [0.25] * 70,                      # one CTA per SM (more than 64 layers); fp64: 18 warps
     "period2x4": [1.0, 0.5] * 4,                 # [A/B]x4 multilayer: generic classes
     "period3x6": [1.0, 0.25, 2.0] * 6,           # 18 layers: generic classes, 4 targets per warp
     "saf": [5.0, 1.0, 5.0, 1.0, 3.0],            # one coincidence only: automatic mode leaves it off
@@ -64,17 +65,27 @@ def test_dedup_field_matches_oracle(hb, stack, prec):
     m = w.m_rounded()
     plan, H = _field(hb, w, m, dedup=2)
     info = hb.plan_info(plan.handle)
-    assert info.n_classes == _expected_classes(dz)
     if stack.startswith("equal"):
-        assert info.n_classes == 2 * nz - 1 and info.dedup == 3
+        # 2nz-1 distinct tensors, folded to |i-j| (N_ji = N_ij up to the sign of xz, yz)
+        assert _expected_classes(dz) == 2 * nz - 1 and info.n_classes == nz
+        assert info.dedup == (3 if nz <= 64 or prec == "f32" else 1)
     else:
-        assert info.dedup == 2
+        assert info.n_classes == _expected_classes(dz) and info.dedup == 2
     assert info.bank_bytes == 6 * info.n_classes * info.n_k_padded * (4 if prec == "f32" else 8)
     ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
     assert _relerr(H, ref) <= TOL[prec]
     # automatic mode: on iff at most half of the pairs carry their own tensor
     auto = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, dz, prec)
     assert (hb.plan_info(auto.handle).dedup != 0) == (2 * info.n_classes <= nz * nz)
+    if stack.startswith("equal"):
+        # the folded bank reproduces the plain bank pair by pair (signs of xz, yz for i < j included)
+        plain = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, dz, prec, dedup=0)
+        plain.build_tensor()
+        for (i, j) in [(0, nz - 1), (nz - 1, 0), (1, 3), (3, 1), (2, 2)]:
+            for c in range(6):
+                x, y = hb.read_bank(plain.handle, i, j, c), hb.read_bank(plan.handle, i, j, c)
+                assert np.abs(x - y).max() <= 1e-13 * max(np.abs(x).max(), 1e-30)
+        plain.close()
     auto.close()
     plan.close()
 
@@ -112,7 +123,7 @@ def test_dedup_on_a_stack_without_duplicates(hb):
     p2.close()
 
 
-@pytest.mark.parametrize("prec,nz", [("f64", 50), ("f32", 100)])
+@pytest.mark.parametrize("prec,nz", [("f64", 80), ("f32", 100)])
 def test_dedup_streaming_kernel_when_the_tile_does_not_fit(hb, prec, nz):
     """Equal thicknesses with too many layers for the shared-memory kernel: class-indexed streaming kernel."""
     dz = np.full(nz, 0.5)
@@ -120,7 +131,7 @@ def test_dedup_streaming_kernel_when_the_tile_does_not_fit(hb, prec, nz):
     m = w.m_rounded()
     plan, H = _field(hb, w, m, dedup=1)
     info = hb.plan_info(plan.handle)
-    assert info.dedup == 1 and info.n_classes == 2 * nz - 1
+    assert info.dedup == 1 and info.n_classes == nz
     ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
     assert _relerr(H, ref) <= TOL[prec]
     plan.close()
