@@ -236,7 +236,9 @@ def main():
     Ms = w.Ms
     nbytes = m.numel() * m.element_size()
     dedup = int(plan.info.dedup)
-    ab = algorithmic_bytes(w, plan.info.n_classes if dedup else None)
+    # bank slots per wavevector: nz^2 pairs, tensor classes, or the Lz values of kz in the z-FFT mode
+    slots = int(plan.info.bank_bytes // (6 * plan.info.n_k_padded * (4 if w.precision == "f32" else 8)))
+    ab = algorithmic_bytes(w, slots if dedup else None)
     # inputs larger than L2?  otherwise flush L2 between steps (and say so)
     flush = None
     if ab["whole"] < 512 << 20:
@@ -340,7 +342,9 @@ def main():
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
             "setup_s": setup_s,
         }
-        if dedup >= 2:
+        if dedup == 4:
+            line["roofline"]["kernel"] = "coupling_zfft_kernel (S3, z-convolution by FFT, PAPER.md:182 Eq.25)"
+        if dedup in (2, 3):
             # deduplicated bank held in shared memory: the coupling is bound by the FP32/FP64 FMA pipe, not by HBM
             # (18 nz^2 n_k B real FMAs; peak = SMs x 128 (fp32) or 64 (fp64) FMA lanes x 2 x clock)
             flops = 2.0 * 18 * w.nz * w.nz * (2 * w.ny * (w.nx + 1)) * w.B
@@ -353,7 +357,7 @@ def main():
                                 "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
                                 "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
                                 "hbm_gbs": achieved, "traffic": None}
-        line["config"]["bank"] = {"dedup": dedup, "slots_per_k": int(plan.info.n_classes if dedup else w.nz * w.nz),
+        line["config"]["bank"] = {"dedup": dedup, "slots_per_k": slots,
                                   "bytes": int(plan.info.bank_bytes)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)

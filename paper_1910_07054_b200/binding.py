@@ -115,7 +115,7 @@ def plan_set_batch(plan, batch):
 
 
 def plan_set_dedup(plan, mode):
-    """0 off, 1 automatic (default), 2 on."""
+    """0 off, 1 automatic (default), 2 on, 3 z-FFT method (equal thicknesses; Eq.25)."""
     _check(lib().hfft_plan_set_dedup(plan, int(mode)), plan)
 
 

@@ -491,6 +491,7 @@ static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
 template <typename T>
 cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
     constexpr int KV = 16 / sizeof(T);
+    if (a.zfft) return launch_coupling_zfft<T>(a, st);
     if (a.cls) {
         if (a.class_kernel) return a.tile_k == 32 ? launch_coupling_class<T>(a, st) : cudaErrorInvalidValue;
         if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, true>(a, st);

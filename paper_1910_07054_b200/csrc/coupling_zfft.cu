@@ -1,0 +1,273 @@
+// coupling_zfft.cu -- stage S3 for stacks of EQUAL layer thickness by the method the paper compares
+// against: the z-convolution is also done by FFT, Eq.25
+//
+//     H = - F3^-1 [ F3(N) F3(M) ],
+//
+// here with the in-plane transforms already done by S1/S2 (and undone by S4/S5), so that S3 is, per
+// in-plane wavevector k and component, a zero-padded FFT of length Lz >= 2 nz along z, a real
+// symmetric 3 x 3 multiply per (k, kz), and the inverse FFT cropped to the nz layers:
+// O(nz log nz) per wavevector instead of the O(nz^2) of the explicit sum.
+//
+// Bank (zdft_bank_kernel, setup): with g_d the in-plane spectra of the Toeplitz classes d = i - j
+// (real a^c_d for xx, yy, zz, xy, even in d; i a^c_d for xz, yz, odd in d; the factor -1/(4 nx ny)
+// folded, tensor_build.cu), on the periodic grid of length Lz (slot d = Lz/2 unused = 0):
+//     S^c(kz) = [ a^c_0 + 2 sum_{d>0} a^c_d cos(2 pi kz d / Lz) ] / Lz      c = xx, yy, zz, xy
+//     S^c(kz) = [         2 sum_{d>0} a^c_d sin(2 pi kz d / Lz) ] / Lz      c = xz, yz   (i * (-i) = 1)
+// all real: H^(k, kz) = S(k, kz) M^(k, kz) with S the symmetric matrix [[xx,xy,xz],[xy,yy,yz],[xz,yz,zz]]
+// acting on the UNROTATED spectra (S2 / S4 run with nz_rot = 0 in this mode).
+// Layout [tile][kz][6][32] in the plan precision: every value is read once per evaluation, straight
+// from global memory (128 B per warp), 6 Lz reals per wavevector.
+//
+// Kernel: lane = wavevector (global accesses are 256 B per warp along k), warp t of the TT warps of
+// a CTA owns the layers n = t + TT q, q < E (Lz = E TT).  Forward (decimation in frequency):
+//     Y[t][r] = W_Lz^{t r} sum_q x[t + TT q] W_E^{q r}          in registers (upper half of q is zero)
+//     X[r + E s] = sum_t Y[t][r] W_TT^{t s}                     after ONE exchange through shared memory
+// (thread t' takes r = t' E/TT ... and all t), multiply, and the same two steps backwards.
+#include "hfft_internal.h"
+#include "fft.cuh"
+
+namespace hfft {
+
+// DFT of N <= 16 points in registers, natural order in and out; ZH: v[N/2 ..] are zero on entry
+template <int N, bool INV, bool ZH, typename T, typename C>
+__device__ __forceinline__ void rdft(C* v) {
+    if constexpr (N == 2) dft2<INV, ZH>(v[0], v[1]);
+    else if constexpr (N == 4) dft4<INV, ZH>(v[0], v[1], v[2], v[3]);
+    else if constexpr (N == 8) dft8<INV, ZH, T>(v[0], v[1], v[2], v[3], v[4], v[5], v[6], v[7]);
+    else if constexpr (N == 16) {
+        // X[2m] = DFT8(a_n + a_{n+8})[m], X[2m+1] = DFT8((a_n - a_{n+8}) W16^n)[m]
+        const T c1 = (T)0.92387953251128675613, s1 = (T)0.38268343236508977173, h = (T)0.70710678118654752440;
+        C e[8], o[8];
+#pragma unroll
+        for (int n = 0; n < 8; ++n) {
+            if (ZH) { e[n] = v[n]; o[n] = v[n]; }
+            else { e[n] = cadd(v[n], v[n + 8]); o[n] = csub(v[n], v[n + 8]); }
+        }
+        o[1] = tmul<INV>(o[1], mk<T>(c1, -s1));
+        o[2] = tmul<INV>(o[2], mk<T>(h, -h));
+        o[3] = tmul<INV>(o[3], mk<T>(s1, -c1));
+        o[4] = mul_qt<INV>(o[4]);
+        o[5] = tmul<INV>(o[5], mk<T>(-s1, -c1));
+        o[6] = tmul<INV>(o[6], mk<T>(-h, -h));
+        o[7] = tmul<INV>(o[7], mk<T>(-c1, -s1));
+        dft8<INV, false, T>(e[0], e[1], e[2], e[3], e[4], e[5], e[6], e[7]);
+        dft8<INV, false, T>(o[0], o[1], o[2], o[3], o[4], o[5], o[6], o[7]);
+#pragma unroll
+        for (int m = 0; m < 8; ++m) { v[2 * m] = e[m]; v[2 * m + 1] = o[m]; }
+    }
+}
+
+template <int LOG2LZ> struct ZCfg {
+    static constexpr int LZ = 1 << LOG2LZ;
+    static constexpr int LOG2E = LOG2LZ <= 3 ? LOG2LZ : (LOG2LZ + 1) / 2;
+    static constexpr int E = 1 << LOG2E;          // layers per thread (registers)
+    static constexpr int TT = LZ / E;             // warps per CTA
+    static constexpr int RPT = E / TT;            // r values per thread after the exchange (E >= TT)
+};
+
+template <typename T, int LOG2LZ>
+__global__ void __launch_bounds__(32 * ZCfg<LOG2LZ>::TT)
+coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, const HFFT_C* __restrict__ twz, int nz,
+                     int batch, long long n_tiles, long long ks) {
+    typedef HFFT_C C;
+    typedef ZCfg<LOG2LZ> Z;
+    constexpr int LZ = Z::LZ, E = Z::E, TT = Z::TT, RPT = Z::RPT, TK = 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* ex = reinterpret_cast<C*>(smem_raw);                    // [3][LZ][32] (TT > 1)
+    C* stw = ex + (TT > 1 ? 3 * LZ * TK : 0);                  // [LZ] exp(-2 pi i n / LZ)
+    const int lane = threadIdx.x & 31, t = threadIdx.x >> 5;
+    const int np = 3 * nz;
+    for (int x = threadIdx.x; x < LZ; x += blockDim.x) stw[x] = twz[x];
+    __syncthreads();
+
+    const long long n_items = n_tiles * batch;
+    for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const long long tile = item / batch;
+        const int b = (int)(item - tile * batch);
+        C* sp = spec + (long long)b * np * ks + tile * TK + lane;
+        C v[3][E];
+        // ---- forward: DFT_E over q (upper half zero), twiddle W_LZ^{t r} ----
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {
+                const int n = t + TT * q;
+                v[c][q] = n < nz ? sp[(long long)(c * nz + n) * ks] : mk<T>((T)0, (T)0);
+            }
+            rdft<E, false, true, T>(v[c]);
+        }
+        if constexpr (TT > 1) {
+#pragma unroll
+            for (int r = 1; r < E; ++r) {
+                const C w = stw[(t * r) & (LZ - 1)];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) v[c][r] = cmul(v[c][r], w);
+            }
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int r = 0; r < E; ++r) ex[((c * LZ) + r * TT + t) * TK + lane] = v[c][r];
+            __syncthreads();
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr)
+#pragma unroll
+                    for (int s = 0; s < TT; ++s) v[c][rr * TT + s] = ex[((c * LZ) + (t * RPT + rr) * TT + s) * TK + lane];
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) rdft<TT, false, false, T>(&v[c][rr * TT]);
+        }
+        // ---- v[c][rr TT + s] = M^_c(k, kz), kz = r + E s, r = t RPT + rr: multiply by S(k, kz) ----
+        const T* bt = bank3 + tile * LZ * (6LL * TK) + lane;
+#pragma unroll
+        for (int rr = 0; rr < RPT; ++rr)
+#pragma unroll
+            for (int s = 0; s < TT; ++s) {
+                const int kz = (TT > 1 ? t * RPT + rr : rr) + E * s;
+                T a[6];
+#pragma unroll
+                for (int c = 0; c < 6; ++c) a[c] = __ldcs(bt + (kz * 6 + c) * TK);
+                const int o = rr * TT + s;
+                const C mx = v[0][o], my = v[1][o], mz = v[2][o];
+                C hx = cscale(a[0], mx), hy = cscale(a[3], mx), hz = cscale(a[4], mx);
+                hx = caxpy(a[3], my, hx); hy = caxpy(a[1], my, hy); hz = caxpy(a[5], my, hz);
+                hx = caxpy(a[4], mz, hx); hy = caxpy(a[5], mz, hy); hz = caxpy(a[2], mz, hz);
+                v[0][o] = hx; v[1][o] = hy; v[2][o] = hz;
+            }
+        // ---- inverse ----
+        if constexpr (TT > 1) {
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr) rdft<TT, true, false, T>(&v[c][rr * TT]);
+            __syncthreads();                                   // everyone has read the forward exchange
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int rr = 0; rr < RPT; ++rr)
+#pragma unroll
+                    for (int s = 0; s < TT; ++s) ex[((c * LZ) + (t * RPT + rr) * TT + s) * TK + lane] = v[c][rr * TT + s];
+            __syncthreads();
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int r = 0; r < E; ++r) v[c][r] = ex[((c * LZ) + r * TT + t) * TK + lane];
+#pragma unroll
+            for (int r = 1; r < E; ++r) {
+                const C w = stw[(t * r) & (LZ - 1)];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) v[c][r] = cmulc(v[c][r], w);
+            }
+        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            rdft<E, true, false, T>(v[c]);
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {                  // crop: layers n < nz <= LZ / 2
+                const int n = t + TT * q;
+                if (n < nz) sp[(long long)(c * nz + n) * ks] = v[c][q];
+            }
+        }
+        if constexpr (TT > 1) __syncthreads();                 // the exchange buffer is free again
+    }
+}
+
+// ---- setup: z-DFT of the Toeplitz classes ----
+// cls64: [nz][6][kstride] fp64 (class d = i - j >= 0, plain layout); twz64: exp(-2 pi i n / LZ)
+template <typename T>
+__global__ void __launch_bounds__(128)
+zdft_bank_kernel(T* __restrict__ bank3, const double* __restrict__ cls64, const double2* __restrict__ twz64, int nz,
+                 int LZ, long long n_k, long long kstride, long long n_k_padded) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int kz = blockIdx.y;
+    if (k >= n_k_padded) return;
+    double acc[6] = {0, 0, 0, 0, 0, 0};
+    if (k < n_k) {
+        for (int d = 0; d < nz; ++d) {
+            const double2 w = twz64[(kz * d) & (LZ - 1)];          // (cos, -sin) of 2 pi kz d / LZ
+            const double wc = d == 0 ? 1.0 : 2.0 * w.x, ws = d == 0 ? 0.0 : -2.0 * w.y;
+#pragma unroll
+            for (int c = 0; c < 6; ++c) {
+                const double a = cls64[((size_t)d * 6 + c) * kstride + k];
+                acc[c] += a * (c < 4 ? wc : ws);
+            }
+        }
+    }
+    const long long tile = k / 32;
+    const int kk = (int)(k - tile * 32);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) bank3[((tile * LZ + kz) * 6 + c) * 32 + kk] = (T)(acc[c] / LZ);
+}
+
+cudaError_t launch_zdft_bank(void* bank3, const double* cls64, const void* twz64, int nz, int log2lz, long long n_k,
+                             long long kstride, long long n_k_padded, int prec, cudaStream_t st) {
+    const int LZ = 1 << log2lz;
+    dim3 grid((unsigned)((n_k_padded + 127) / 128), LZ);
+    if (prec == HFFT_F32)
+        zdft_bank_kernel<float><<<grid, 128, 0, st>>>((float*)bank3, cls64, (const double2*)twz64, nz, LZ, n_k, kstride,
+                                                      n_k_padded);
+    else
+        zdft_bank_kernel<double><<<grid, 128, 0, st>>>((double*)bank3, cls64, (const double2*)twz64, nz, LZ, n_k,
+                                                       kstride, n_k_padded);
+    return cudaGetLastError();
+}
+
+// fp32: Lz <= 256 (16 layers x 3 components per thread in registers); fp64: Lz <= 64
+bool coupling_zfft_applies(int nz, size_t elem, int* log2lz) {
+    int l = 1;
+    while ((1 << l) < 2 * nz) ++l;
+    if (log2lz) *log2lz = l;
+    return nz >= 2 && l <= (elem == 4 ? 8 : 6);
+}
+
+template <typename T, int L>
+static cudaError_t launch_zfft_l(const CouplingArgs& a, cudaStream_t st) {
+    typedef HFFT_C C;
+    typedef ZCfg<L> Z;
+    auto kern = coupling_zfft_kernel<T, L>;
+    const size_t smem = ((Z::TT > 1 ? (size_t)3 * Z::LZ * 32 : 0) + Z::LZ) * sizeof(C);
+    const int threads = 32 * Z::TT;
+    static int occ = 0;
+    cudaError_t err;
+    if (occ == 0) {
+        if (smem > 48 * 1024) {
+            err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (err != cudaSuccess) return err;
+        }
+        int nb = 0;
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
+        if (err != cudaSuccess) return err;
+        if (nb < 1) return cudaErrorInvalidConfiguration;
+        occ = nb;
+    }
+    const long long items = a.n_tiles * a.batch;
+    long long grid = (long long)a.num_sms * occ;
+    if (grid > items) grid = items;
+    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, (const C*)a.twz, a.nz, a.batch, a.n_tiles,
+                                                a.ks);
+    return cudaGetLastError();
+}
+
+template <typename T>
+cudaError_t launch_coupling_zfft(const CouplingArgs& a, cudaStream_t st) {
+    switch (a.log2lz) {
+        case 2: return launch_zfft_l<T, 2>(a, st);
+        case 3: return launch_zfft_l<T, 3>(a, st);
+        case 4: return launch_zfft_l<T, 4>(a, st);
+        case 5: return launch_zfft_l<T, 5>(a, st);
+        case 6: return launch_zfft_l<T, 6>(a, st);
+        default: break;
+    }
+    if constexpr (sizeof(T) == 4) {
+        if (a.log2lz == 7) return launch_zfft_l<T, 7>(a, st);
+        if (a.log2lz == 8) return launch_zfft_l<T, 8>(a, st);
+    }
+    return cudaErrorInvalidValue;
+}
+
+template cudaError_t launch_coupling_zfft<float>(const CouplingArgs&, cudaStream_t);
+template cudaError_t launch_coupling_zfft<double>(const CouplingArgs&, cudaStream_t);
+
+}  // namespace hfft

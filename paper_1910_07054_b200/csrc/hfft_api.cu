@@ -33,8 +33,11 @@ struct hfft_plan {
     void *tw_x64 = nullptr, *twt_x64 = nullptr, *twt_y64 = nullptr;
     double* sums = nullptr;                          // hfft_plan_set_reduction: [B][3][nz][2] on device
     // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
-    int dedup_mode = 1;                              // 0 off, 1 auto, 2 on
+    int dedup_mode = 1;                              // 0 off, 1 auto, 2 on, 3 z-FFT (Eq.25)
     bool dedup = false, toeplitz = false, class_kernel = false;
+    bool zfft = false;                               // equal thicknesses: z-convolution by FFT (coupling_zfft.cu)
+    int log2lz = 0;
+    void* d_twz = nullptr;                           // exp(-2 pi i n / Lz), plan precision
     int n_classes = 0;                               // distinct tensors among the nz^2 pairs
     std::vector<int> pair_class, class_rep;
     unsigned short* d_cls = nullptr;                 // device copy of pair_class (dedup only)
@@ -145,17 +148,24 @@ static void plan_sizes(hfft_plan* p) {
     p->n_k = 2LL * p->ny * (p->nx + 1);
     // deduplicated bank: automatically once at most half of the pairs carry a tensor of their own
     p->dedup = p->dedup_mode == 2 || (p->dedup_mode == 1 && 2 * p->n_classes <= p->nz * p->nz);
-    p->class_kernel = p->dedup && coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
+    // equal thicknesses: the z-convolution by FFT (Eq.25) where it applies, from 16 layers on
+    // (below that the explicit Toeplitz sum does less work)
+    p->zfft = p->toeplitz && coupling_zfft_applies(p->nz, e, &p->log2lz) &&
+              (p->dedup_mode == 3 || (p->dedup_mode == 1 && p->nz >= 16));
+    if (p->zfft) p->dedup = true;
+    p->class_kernel = p->dedup && !p->zfft &&
+                      coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
     // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
     const int wide = 32 * (int)(16 / e);
     p->tile_k = (p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148)) ? wide : 32;
     while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
     if (p->tile_k != wide) p->tile_k = 32;
     if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
-    if (p->class_kernel) p->tile_k = 32;
+    if (p->class_kernel || p->zfft) p->tile_k = 32;
     p->n_tiles = (p->n_k + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
-    p->bank_bytes = (size_t)6 * (p->dedup ? p->n_classes : p->nz * p->nz) * (size_t)p->n_k_padded * e;
+    const size_t slots = p->zfft ? ((size_t)1 << p->log2lz) : (p->dedup ? p->n_classes : p->nz * p->nz);
+    p->bank_bytes = (size_t)6 * slots * (size_t)p->n_k_padded * e;
     const size_t planes = (size_t)3 * p->nz * p->batch;
     auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
     size_t o = 0;
@@ -227,8 +237,12 @@ hfft_status hfft_plan_set_batch(hfft_plan* plan, int batch) {
 
 hfft_status hfft_plan_set_dedup(hfft_plan* plan, int mode) {
     if (!plan) return HFFT_EINVAL;
-    if (mode < 0 || mode > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_dedup: mode must be 0, 1 or 2");
+    if (mode < 0 || mode > 3) return fail(plan, HFFT_EINVAL, "hfft_plan_set_dedup: mode must be 0, 1, 2 or 3");
     if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_dedup: after build / set_buffers");
+    if (mode == 3 && !(plan->toeplitz && coupling_zfft_applies(plan->nz, plan->elem, nullptr)))
+        return fail(plan, HFFT_EUNSUPPORTED,
+                    "hfft_plan_set_dedup: the z-FFT method (mode 3) needs equal layer thicknesses, nz >= 2 and "
+                    "nz <= 128 (fp32) / 32 (fp64)");
     plan->dedup_mode = mode;
     plan_sizes(plan);
     return HFFT_OK;
@@ -245,7 +259,7 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
     info->n_classes = plan->n_classes;
-    info->dedup = plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0;
+    info->dedup = plan->zfft ? 4 : (plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0);
     return HFFT_OK;
 }
 
@@ -301,7 +315,30 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     if ((e = cudaMalloc(&scratch, sb)) != cudaSuccess)
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
     std::string msg;
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, -1, st, msg);
+    if (!plan->zfft) {
+        e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, -1, st, msg);
+    } else {
+        // Toeplitz classes in fp64, plain layout [d][6][n_k_padded] (one "tile" of n_k_padded wavevectors), then their
+        // z-DFT into the bank S(k, kz)
+        const int LZ = 1 << plan->log2lz;
+        void *cls64 = nullptr, *twz64 = nullptr;
+        BuildGeom g2 = g;
+        g2.prec = HFFT_F64;
+        g2.tile_k = (int)plan->n_k_padded;
+        e = cudaMalloc(&cls64, (size_t)plan->nz * 6 * plan->n_k_padded * sizeof(double));
+        if (e == cudaSuccess) e = upload_twiddles(LZ, false, &twz64);
+        if (e == cudaSuccess && !plan->d_twz) e = upload_twiddles(LZ, plan->prec == HFFT_F32, &plan->d_twz);
+        if (e != cudaSuccess) msg = std::string("z-FFT setup buffers: ") + cudaGetErrorString(e);
+        if (e == cudaSuccess) e = build_bank(g2, cls64, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, -1, st, msg);
+        if (e == cudaSuccess) {
+            e = launch_zdft_bank(plan->bank, (const double*)cls64, twz64, plan->nz, plan->log2lz, plan->n_k,
+                                 plan->n_k_padded, plan->n_k_padded, plan->prec, st);
+            if (e != cudaSuccess) msg = std::string("zdft_bank_kernel: ") + cudaGetErrorString(e);
+        }
+        cudaStreamSynchronize(st);
+        if (cls64) cudaFree(cls64);
+        if (twz64) cudaFree(twz64);
+    }
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
     if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_build_tensor: " + msg);
@@ -329,13 +366,16 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
     if ((e = (call)) != cudaSuccess) return fail_cuda(p, #call, e);
     STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, p->twt_x,
                                        p->num_sms, st)))
-    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y,
+    // the z components are rotated by i on the k side (real form R6) except in the z-FFT mode
+    const int nz_rot = p->zfft ? 0 : p->nz;
+    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y,
                                        p->num_sms, st)))
-    const CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
-                          p->dedup ? p->n_classes : p->nz * p->nz, p->dedup ? p->d_cls : nullptr,
-                          p->class_kernel, p->toeplitz, p->num_sms};
+    CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
+                    p->dedup ? p->n_classes : p->nz * p->nz, p->dedup ? p->d_cls : nullptr,
+                    p->class_kernel, p->toeplitz, p->num_sms};
+    ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz;
     STAGE(2, (launch_coupling<T>(ca, st)))
-    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, p->nz, p->n_k_padded, p->twt_y, p->num_sms, st)))
+    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st)))
     if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
         return fail_cuda(p, "cudaMemsetAsync(sums)", e);
     STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, (const T*)m,
@@ -446,6 +486,7 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     hfft_plan* p = const_cast<hfft_plan*>(plan);
     if (i < 0 || i >= p->nz || j < 0 || j >= p->nz || c < 0 || c > 5) return fail(p, HFFT_EINVAL, "hfft_read_bank: index out of range");
     if (!p->built) return fail(p, HFFT_ESTATE, "hfft_read_bank: tensor not built");
+    if (p->zfft) return fail(p, HFFT_EUNSUPPORTED, "hfft_read_bank: the bank of the z-FFT mode holds S(k, kz), not N_ij(k)");
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return fail_cuda(p, "cudaDeviceSynchronize", e);
     const int tk = p->tile_k;
@@ -475,6 +516,7 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (plan->tw_x != plan->tw_x64) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
     cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
     if (plan->d_cls) cudaFree(plan->d_cls);
+    if (plan->d_twz) cudaFree(plan->d_twz);
     for (auto& ev : plan->prof_events) cudaEventDestroy(ev);
     delete plan;
     return HFFT_OK;

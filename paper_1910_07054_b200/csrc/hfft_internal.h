@@ -44,11 +44,23 @@ struct CouplingArgs {
     int n_classes;                 // nz*nz without deduplication
     const unsigned short* cls;     // device, [nz*nz], or nullptr
     bool class_kernel;             // bank tile in shared memory (coupling_class_applies)
-    bool toeplitz;                 // cls[i*nz+j] == i - j + nz - 1
+    bool toeplitz;                 // equal thicknesses: cls[i*nz+j] == |i - j|, xz / yz negated for i < j
     int num_sms;
+    // z-FFT mode (coupling_zfft.cu; Eq.25): bank = S(k, kz) [tile][kz][6][32], Lz = 2^log2lz
+    bool zfft = false;
+    int log2lz = 0;
+    const void* twz = nullptr;     // device, exp(-2 pi i n / Lz), plan precision
 };
 template <typename T>
 cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st);
+// ---- coupling_zfft.cu ----
+template <typename T>
+cudaError_t launch_coupling_zfft(const CouplingArgs& a, cudaStream_t st);
+bool coupling_zfft_applies(int nz, size_t elem, int* log2lz);
+// bank3 [tile][kz][6][32] (plan precision) from the fp64 Toeplitz classes cls64 [nz][6][kstride]
+cudaError_t launch_zdft_bank(void* bank3, const double* cls64, const void* twz64, int nz, int log2lz, long long n_k,
+                             long long kstride, long long n_k_padded, int prec, cudaStream_t st);
+
 // shared-memory-resident class kernel: needs tile_k == 32 and this many bytes per CTA
 size_t coupling_class_smem_bytes(int nz, int n_classes, bool toeplitz, size_t elem);
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem);

@@ -129,7 +129,7 @@ def test_dedup_streaming_kernel_when_the_tile_does_not_fit(hb, prec, nz):
     dz = np.full(nz, 0.5)
     w = W.small(8, 8, nz, precision=prec, seed=nz, dz=dz)
     m = w.m_rounded()
-    plan, H = _field(hb, w, m, dedup=1)
+    plan, H = _field(hb, w, m, dedup=2)
     info = hb.plan_info(plan.handle)
     assert info.dedup == 1 and info.n_classes == nz
     ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
@@ -153,7 +153,7 @@ def test_dedup_errors(hb):
     dz = np.ones(6)
     p = hb.Plan(8, 8, 6, 1.0, 1.0, dz, "f64")
     with pytest.raises(hb.HfftError) as e:
-        hb.plan_set_dedup(p.handle, 3)
+        hb.plan_set_dedup(p.handle, 4)
     assert e.value.status == hb.EINVAL
     with pytest.raises(hb.HfftError) as e:          # buffers already handed over: sizes are fixed
         hb.plan_set_dedup(p.handle, 0)
@@ -168,3 +168,74 @@ def test_dedup_errors(hb):
     q.build_tensor()
     q.update_dz(2, 1.5)                              # allowed on the plain bank
     q.close()
+
+
+# ---- z-FFT mode (mode 3): the equidistant 3-D FFT method of PAPER.md:182 Eq.25 as stage S3 ----
+ZFFT_NZ = [2, 3, 4, 5, 8, 12, 16, 17, 32, 33, 64, 70, 128]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("nz", ZFFT_NZ)
+def test_zfft_field_matches_oracle(hb, nz, prec):
+    if prec == "f64" and nz > 32:
+        pytest.skip("fp64 z-FFT kernel: Lz <= 64")
+    dz = np.full(nz, 0.75)
+    nx, ny = (16, 8) if nz <= 33 else (8, 8)
+    w = W.small(nx, ny, nz, precision=prec, seed=400 + nz, dz=dz)
+    m = w.m_rounded()
+    plan, H = _field(hb, w, m, dedup=3)
+    info = hb.plan_info(plan.handle)
+    lz = 1
+    while lz < 2 * nz:
+        lz *= 2
+    assert info.dedup == 4
+    assert info.bank_bytes == 6 * lz * info.n_k_padded * (4 if prec == "f32" else 8)
+    ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    if nx * ny * nz <= 2048:
+        ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, dz, m[0], w.Ms)     # the definition, Eq.18
+        assert _relerr(H[0], ref0) <= TOL[prec]
+    # automatic mode picks the z-FFT from 16 equal layers on
+    auto = hb.Plan(nx, ny, nz, w.dx, w.dy, dz, prec)
+    assert (hb.plan_info(auto.handle).dedup == 4) == (nz >= 16)
+    auto.close()
+    plan.close()
+
+
+def test_zfft_batched_and_reductions(hb):
+    import torch
+    nz, B = 16, 3
+    dz = np.full(nz, 1.25)
+    w = W.small(32, 16, nz, precision="f32", B=B, seed=77, dz=dz)
+    m = w.m_rounded()
+    plan = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, dz, "f32", batch=B, dedup=3)
+    plan.build_tensor()
+    sums = plan.set_reduction(True)
+    H = plan.demag(torch.from_numpy(m).float().cuda(), w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f32"]
+    got = sums.cpu().numpy()[..., 0]
+    assert np.abs(got - ref.sum(axis=(-1, -2))).max() <= TOL["f32"] * np.abs(ref).max() * w.nx * w.ny
+    plan.close()
+
+
+def test_zfft_errors(hb):
+    p = hb.Plan(8, 8, 4, 1.0, 1.0, np.array([1.0, 2.0, 1.0, 1.0]), "f32", torch_buffers=False)
+    with pytest.raises(hb.HfftError) as e:          # unequal thicknesses
+        hb.plan_set_dedup(p.handle, 3)
+    assert e.value.status == hb.EUNSUPPORTED
+    p.close()
+    q = hb.Plan(8, 8, 40, 1.0, 1.0, np.ones(40), "f64", torch_buffers=False)
+    with pytest.raises(hb.HfftError) as e:          # fp64: Lz <= 64
+        hb.plan_set_dedup(q.handle, 3)
+    assert e.value.status == hb.EUNSUPPORTED
+    q.close()
+    r = hb.Plan(8, 8, 4, 1.0, 1.0, np.ones(4), "f64", dedup=3)
+    r.build_tensor()
+    with pytest.raises(hb.HfftError) as e:
+        hb.read_bank(r.handle, 0, 0, 0)
+    assert e.value.status == hb.EUNSUPPORTED
+    with pytest.raises(hb.HfftError) as e:
+        r.update_dz(1, 2.0)
+    assert e.value.status == hb.EUNSUPPORTED
+    r.close()
