@@ -65,22 +65,63 @@ template <int LOG2LZ> struct ZCfg {
     static constexpr int RPT = E / TT;            // r values per thread after the exchange (E >= TT)
 };
 
+// STAGE: the S tile of an item ([LZ][6][32] reals, contiguous in the bank) is copied to shared memory by cp.async
+// while the previous item finishes and this item's forward transform runs, so the multiply never waits for HBM
+// (ncu on the register-only version: long-scoreboard stalls on the bank loads dominate).  Used where the
+// exchange buffer and the tile fit together (fp32: Lz <= 128, fp64: Lz <= 64).
+template <typename T, int LOG2LZ> struct ZOcc {
+    typedef typename cplx_of<T>::type C;
+    static constexpr int LZ = ZCfg<LOG2LZ>::LZ, TT = ZCfg<LOG2LZ>::TT;
+    static constexpr int THREADS = 32 * TT;
+    static constexpr size_t EX_BYTES = TT > 1 ? (size_t)3 * LZ * 32 * sizeof(C) : 0;
+    static constexpr size_t BANK_BYTES = (size_t)LZ * 6 * 32 * sizeof(T);
+    static constexpr bool STAGE = TT > 1 && EX_BYTES + BANK_BYTES + LZ * sizeof(C) <= 200 * 1024;
+    static constexpr size_t SMEM = EX_BYTES + (STAGE ? BANK_BYTES : 0) + LZ * sizeof(C);
+};
+
+// multiply the three components at one (k, kz) by the real symmetric S(k, kz); bt: shared or global
+template <bool SMEM, typename T, typename C>
+__device__ __forceinline__ void zmul(const T* __restrict__ bt, C& x, C& y, C& z) {
+    T a[6];
+#pragma unroll
+    for (int c = 0; c < 6; ++c) a[c] = SMEM ? bt[c * 32] : __ldcs(bt + c * 32);
+    const C mx = x, my = y, mz = z;
+    C hx = cscale(a[0], mx), hy = cscale(a[3], mx), hz = cscale(a[4], mx);
+    hx = caxpy(a[3], my, hx); hy = caxpy(a[1], my, hy); hz = caxpy(a[5], my, hz);
+    hx = caxpy(a[4], mz, hx); hy = caxpy(a[5], mz, hy); hz = caxpy(a[2], mz, hz);
+    x = hx; y = hy; z = hz;
+}
+
 template <typename T, int LOG2LZ>
-__global__ void __launch_bounds__(32 * ZCfg<LOG2LZ>::TT)
+__global__ void __launch_bounds__(ZOcc<T, LOG2LZ>::THREADS)
 coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, const HFFT_C* __restrict__ twz, int nz,
                      int batch, long long n_tiles, long long ks) {
     typedef HFFT_C C;
     typedef ZCfg<LOG2LZ> Z;
+    typedef ZOcc<T, LOG2LZ> O;
     constexpr int LZ = Z::LZ, E = Z::E, TT = Z::TT, RPT = Z::RPT, TK = 32;
+    constexpr bool STAGE = O::STAGE;
+    constexpr int CHUNK_T = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    C* ex = reinterpret_cast<C*>(smem_raw);                    // [3][LZ][32] (TT > 1)
-    C* stw = ex + (TT > 1 ? 3 * LZ * TK : 0);                  // [LZ] exp(-2 pi i n / LZ)
+    C* ex = reinterpret_cast<C*>(smem_raw);                                   // [3][LZ][32] (TT > 1)
+    T* sbank = reinterpret_cast<T*>(smem_raw + O::EX_BYTES);                   // [LZ][6][32] (STAGE)
+    C* stw = reinterpret_cast<C*>(smem_raw + O::EX_BYTES + (STAGE ? O::BANK_BYTES : 0));   // [LZ] exp(-2 pi i n / LZ)
     const int lane = threadIdx.x & 31, t = threadIdx.x >> 5;
     const int np = 3 * nz;
     for (int x = threadIdx.x; x < LZ; x += blockDim.x) stw[x] = twz[x];
-    __syncthreads();
 
     const long long n_items = n_tiles * batch;
+    auto fetch_bank = [&](long long it) {
+        if (STAGE && it < n_items) {
+            const T* src = bank3 + (it / batch) * LZ * (6LL * TK);
+            for (int x = threadIdx.x; x < LZ * 6 * TK / CHUNK_T; x += blockDim.x)
+                cp_async16(sbank + x * CHUNK_T, src + x * CHUNK_T);
+        }
+        cp_async_commit();
+    };
+    fetch_bank(blockIdx.x);
+    __syncthreads();
+
     for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
         const long long tile = item / batch;
         const int b = (int)(item - tile * batch);
@@ -88,14 +129,14 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
         C v[3][E];
         // ---- forward: DFT_E over q (upper half zero), twiddle W_LZ^{t r} ----
 #pragma unroll
-        for (int c = 0; c < 3; ++c) {
+        for (int c = 0; c < 3; ++c)
 #pragma unroll
             for (int q = 0; q < E / 2; ++q) {
                 const int n = t + TT * q;
                 v[c][q] = n < nz ? sp[(long long)(c * nz + n) * ks] : mk<T>((T)0, (T)0);
             }
-            rdft<E, false, true, T>(v[c]);
-        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c) rdft<E, false, true, T>(v[c]);
         if constexpr (TT > 1) {
 #pragma unroll
             for (int r = 1; r < E; ++r) {
@@ -107,6 +148,7 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int r = 0; r < E; ++r) ex[((c * LZ) + r * TT + t) * TK + lane] = v[c][r];
+            if (STAGE) cp_async_wait_group<0>();               // this thread's part of the S tile has landed
             __syncthreads();
 #pragma unroll
             for (int c = 0; c < 3; ++c)
@@ -120,21 +162,14 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
                 for (int rr = 0; rr < RPT; ++rr) rdft<TT, false, false, T>(&v[c][rr * TT]);
         }
         // ---- v[c][rr TT + s] = M^_c(k, kz), kz = r + E s, r = t RPT + rr: multiply by S(k, kz) ----
-        const T* bt = bank3 + tile * LZ * (6LL * TK) + lane;
+        const T* bt = STAGE ? sbank + lane : bank3 + tile * LZ * (6LL * TK) + lane;
 #pragma unroll
         for (int rr = 0; rr < RPT; ++rr)
 #pragma unroll
             for (int s = 0; s < TT; ++s) {
                 const int kz = (TT > 1 ? t * RPT + rr : rr) + E * s;
-                T a[6];
-#pragma unroll
-                for (int c = 0; c < 6; ++c) a[c] = __ldcs(bt + (kz * 6 + c) * TK);
                 const int o = rr * TT + s;
-                const C mx = v[0][o], my = v[1][o], mz = v[2][o];
-                C hx = cscale(a[0], mx), hy = cscale(a[3], mx), hz = cscale(a[4], mx);
-                hx = caxpy(a[3], my, hx); hy = caxpy(a[1], my, hy); hz = caxpy(a[5], my, hz);
-                hx = caxpy(a[4], mz, hx); hy = caxpy(a[5], mz, hy); hz = caxpy(a[2], mz, hz);
-                v[0][o] = hx; v[1][o] = hy; v[2][o] = hz;
+                zmul<STAGE, T>(bt + kz * 6 * TK, v[0][o], v[1][o], v[2][o]);
             }
         // ---- inverse ----
         if constexpr (TT > 1) {
@@ -142,7 +177,8 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
             for (int c = 0; c < 3; ++c)
 #pragma unroll
                 for (int rr = 0; rr < RPT; ++rr) rdft<TT, true, false, T>(&v[c][rr * TT]);
-            __syncthreads();                                   // everyone has read the forward exchange
+            __syncthreads();                                   // everyone is done with the forward exchange and the S tile
+            fetch_bank(item + gridDim.x);                      // next item's S tile flies from here on
 #pragma unroll
             for (int c = 0; c < 3; ++c)
 #pragma unroll
@@ -172,6 +208,7 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
         }
         if constexpr (TT > 1) __syncthreads();                 // the exchange buffer is free again
     }
+    cp_async_wait_group<0>();
 }
 
 // ---- setup: z-DFT of the Toeplitz classes ----
@@ -227,7 +264,7 @@ static cudaError_t launch_zfft_l(const CouplingArgs& a, cudaStream_t st) {
     typedef HFFT_C C;
     typedef ZCfg<L> Z;
     auto kern = coupling_zfft_kernel<T, L>;
-    const size_t smem = ((Z::TT > 1 ? (size_t)3 * Z::LZ * 32 : 0) + Z::LZ) * sizeof(C);
+    const size_t smem = ZOcc<T, L>::SMEM;
     const int threads = 32 * Z::TT;
     static int occ = 0;
     cudaError_t err;
