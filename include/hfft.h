@@ -61,7 +61,7 @@ typedef struct {
     long long n_k;            /* wavevectors in the Hermitian half spectrum: (nx+1) * 2ny */
     long long n_k_padded;     /* n_k rounded up to a multiple of tile_k */
     size_t bank_bytes;        /* spectral tensor bank: 6 * (nz^2 or n_classes) * n_k_padded * sizeof(element) */
-    size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging */
+    size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging (two slots of m and h) */
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
     int launches_per_demag;   /* kernels hfft_demag enqueues per call */
     int built;                /* 1 once hfft_build_tensor has completed */
@@ -154,6 +154,23 @@ hfft_status hfft_demag(hfft_plan *plan, const void *m, const double *Ms, void *h
  */
 hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *Ms, void *h_host,
                             void *stream);
+
+/*
+ * Pipelined form of hfft_demag_host for back-to-back evaluations (a time loop
+ * feeding magnetisations from the host): the copy-in, the five kernels and the
+ * copy-out run on three streams owned by the plan, with two staging slots, so
+ * the PCIe transfers of evaluation n+1 / n-1 overlap the kernels of evaluation
+ * n.  The call waits (on the device, not on the host) for everything enqueued on
+ * `stream` before it, then returns at once; h_host is valid only after
+ * hfft_host_join(plan, stream) followed by a synchronisation of `stream` (or of
+ * an event recorded on it).  m_host must stay unchanged until then; pinned
+ * memory is needed for the copies to be asynchronous.  Evaluations complete in
+ * call order.  Not capturable in a CUDA graph.  Errors: as hfft_demag_host.
+ */
+hfft_status hfft_demag_host_async(hfft_plan *plan, const void *m_host, const double *Ms, void *h_host,
+                                  void *stream);
+/* Makes `stream` wait for every hfft_demag_host_async issued so far (no host blocking). */
+hfft_status hfft_host_join(hfft_plan *plan, void *stream);
 
 /*
  * Geometry update for layer-thickness optimisation (section 4

@@ -24,7 +24,7 @@ MAX_NZ = 256
 
 # every symbol include/hfft.h declares
 EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_info", "hfft_plan_set_buffers",
-           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_update_dz", "hfft_plan_set_reduction",
+           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
 
@@ -67,6 +67,8 @@ def lib():
         L.hfft_build_tensor.argtypes = [vp, vp]
         L.hfft_demag.argtypes = [vp, vp, dp, vp, vp]
         L.hfft_demag_host.argtypes = [vp, vp, dp, vp, vp]
+        L.hfft_demag_host_async.argtypes = [vp, vp, dp, vp, vp]
+        L.hfft_host_join.argtypes = [vp, vp]
         L.hfft_update_dz.argtypes = [vp, ctypes.c_int, ctypes.c_double, vp]
         L.hfft_plan_set_reduction.argtypes = [vp, vp]
         L.hfft_profile_enable.argtypes = [vp, ctypes.c_int]
@@ -156,6 +158,18 @@ def demag_host(plan, m_host_ptr, Ms, h_host_ptr, stream=0, nz=None):
                                  ctypes.c_void_p(stream)), plan)
 
 
+def demag_host_async(plan, m_host_ptr, Ms, h_host_ptr, stream=0, nz=None):
+    if Ms is not None and nz is None:
+        nz = plan_info(plan).nz
+    keep, p = _ms(Ms, nz)
+    _check(lib().hfft_demag_host_async(plan, ctypes.c_void_p(m_host_ptr), p, ctypes.c_void_p(h_host_ptr),
+                                       ctypes.c_void_p(stream)), plan)
+
+
+def host_join(plan, stream=0):
+    _check(lib().hfft_host_join(plan, ctypes.c_void_p(stream)), plan)
+
+
 def update_dz(plan, k, dz_new, stream=0):
     _check(lib().hfft_update_dz(plan, int(k), float(dz_new), ctypes.c_void_p(stream)), plan)
 
@@ -240,6 +254,18 @@ class Plan:
             h_host = t.empty_like(m_host).pin_memory()
         demag_host(self.handle, m_host.data_ptr(), Ms, h_host.data_ptr(), self._stream(), nz=self.nz)
         return h_host
+
+    def demag_host_async(self, m_host, Ms=None, h_host=None):
+        """Pipelined host path: returns at once; h_host is valid after host_join() + a stream synchronisation."""
+        t = self.torch
+        assert not m_host.is_cuda and m_host.dtype == self.dtype and m_host.is_contiguous()
+        if h_host is None:
+            h_host = t.empty_like(m_host).pin_memory()
+        demag_host_async(self.handle, m_host.data_ptr(), Ms, h_host.data_ptr(), self._stream(), nz=self.nz)
+        return h_host
+
+    def host_join(self):
+        host_join(self.handle, self._stream())
 
     def update_dz(self, k, dz_new):
         update_dz(self.handle, k, dz_new, self._stream())

@@ -25,6 +25,12 @@ struct hfft_plan {
     size_t elem = 4;
     size_t bank_bytes = 0, ws_bytes = 0;
     size_t ws_xhat = 0, ws_spec = 0, ws_stage_m = 0, ws_stage_h = 0;   // offsets into the workspace
+    size_t ws_stage_m2 = 0, ws_stage_h2 = 0;         // second staging pair of the pipelined host path
+    // hfft_demag_host_async: copy-in, compute and copy-out streams, per staging slot events
+    cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_user = nullptr, ev_h2d[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr},
+                ev_d2h[2] = {nullptr, nullptr};
+    unsigned long long pipe_calls = 0;
     void *bank = nullptr, *ws = nullptr;
     bool own_bank = false, own_ws = false, built = false;
     // tw_x: exp(-2 pi i t / 2nx), 2nx entries; twt_x / twt_y: per-thread tables of the length-nx and
@@ -173,6 +179,8 @@ static void plan_sizes(hfft_plan* p) {
     p->ws_spec = o;    o += al(planes * (size_t)p->n_k_padded * 2 * e);
     p->ws_stage_m = o; o += al(planes * (size_t)p->ny * p->nx * e);
     p->ws_stage_h = o; o += al(planes * (size_t)p->ny * p->nx * e);
+    p->ws_stage_m2 = o; o += al(planes * (size_t)p->ny * p->nx * e);
+    p->ws_stage_h2 = o; o += al(planes * (size_t)p->ny * p->nx * e);
     p->ws_bytes = o;
 }
 
@@ -448,6 +456,63 @@ hfft_status hfft_demag_host(hfft_plan* plan, const void* m_host, const double* M
     return HFFT_OK;
 }
 
+static cudaError_t pipe_init(hfft_plan* p) {
+    if (p->s_h2d) return cudaSuccess;
+    cudaError_t e;
+    if ((e = cudaStreamCreateWithFlags(&p->s_h2d, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaStreamCreateWithFlags(&p->s_comp, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    if ((e = cudaStreamCreateWithFlags(&p->s_d2h, cudaStreamNonBlocking)) != cudaSuccess) return e;
+    cudaEvent_t* evs[] = {&p->ev_user, &p->ev_h2d[0], &p->ev_h2d[1], &p->ev_comp[0], &p->ev_comp[1], &p->ev_d2h[0],
+                          &p->ev_d2h[1]};
+    for (cudaEvent_t* ev : evs)
+        if ((e = cudaEventCreateWithFlags(ev, cudaEventDisableTiming)) != cudaSuccess) return e;
+    return cudaSuccess;
+}
+
+hfft_status hfft_demag_host_async(hfft_plan* plan, const void* m_host, const double* Ms, void* h_host, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (!m_host || !h_host) return fail(plan, HFFT_EINVAL, "hfft_demag_host_async: NULL m or h");
+    if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag_host_async: call hfft_build_tensor first");
+    cudaError_t e;
+    if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    if ((e = pipe_init(plan)) != cudaSuccess) return fail_cuda(plan, "hfft_demag_host_async: streams / events", e);
+    unsigned char* ws = static_cast<unsigned char*>(plan->ws);
+    const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
+    const int slot = (int)(plan->pipe_calls & 1);
+    void* dm = ws + (slot ? plan->ws_stage_m2 : plan->ws_stage_m);
+    void* dh = ws + (slot ? plan->ws_stage_h2 : plan->ws_stage_h);
+    const bool reuse = plan->pipe_calls >= 2;        // the slot was used two calls ago
+#define HFFT_PIPE(call) if ((e = (call)) != cudaSuccess) return fail_cuda(plan, "hfft_demag_host_async: " #call, e)
+    // copy-in: after everything the caller enqueued on `stream` so far, and after the evaluation that last read the slot
+    HFFT_PIPE(cudaEventRecord(plan->ev_user, (cudaStream_t)stream));
+    HFFT_PIPE(cudaStreamWaitEvent(plan->s_h2d, plan->ev_user, 0));
+    if (reuse) HFFT_PIPE(cudaStreamWaitEvent(plan->s_h2d, plan->ev_comp[slot], 0));
+    HFFT_PIPE(cudaMemcpyAsync(dm, m_host, bytes, cudaMemcpyHostToDevice, plan->s_h2d));
+    HFFT_PIPE(cudaEventRecord(plan->ev_h2d[slot], plan->s_h2d));
+    // evaluation: after its copy-in, and after the copy-out that last read the slot's h
+    HFFT_PIPE(cudaStreamWaitEvent(plan->s_comp, plan->ev_h2d[slot], 0));
+    if (reuse) HFFT_PIPE(cudaStreamWaitEvent(plan->s_comp, plan->ev_d2h[slot], 0));
+    hfft_status s = hfft_demag(plan, dm, Ms, dh, plan->s_comp);
+    if (s != HFFT_OK) return s;
+    HFFT_PIPE(cudaEventRecord(plan->ev_comp[slot], plan->s_comp));
+    // copy-out
+    HFFT_PIPE(cudaStreamWaitEvent(plan->s_d2h, plan->ev_comp[slot], 0));
+    HFFT_PIPE(cudaMemcpyAsync(h_host, dh, bytes, cudaMemcpyDeviceToHost, plan->s_d2h));
+    HFFT_PIPE(cudaEventRecord(plan->ev_d2h[slot], plan->s_d2h));
+    ++plan->pipe_calls;
+    return HFFT_OK;
+}
+
+hfft_status hfft_host_join(hfft_plan* plan, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (plan->pipe_calls == 0) return HFFT_OK;
+    cudaError_t e;
+    // copy-outs are serialised on one stream: the last one implies all the earlier ones
+    HFFT_PIPE(cudaStreamWaitEvent((cudaStream_t)stream, plan->ev_d2h[(plan->pipe_calls - 1) & 1], 0));
+#undef HFFT_PIPE
+    return HFFT_OK;
+}
+
 hfft_status hfft_profile_enable(hfft_plan* plan, int on) {
     if (!plan) return HFFT_EINVAL;
     if (on && plan->prof_events.empty()) {
@@ -515,6 +580,13 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (plan->own_ws && plan->ws) cudaFree(plan->ws);
     if (plan->tw_x != plan->tw_x64) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
     cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
+    if (plan->s_h2d) {
+        cudaStreamSynchronize(plan->s_h2d); cudaStreamSynchronize(plan->s_comp); cudaStreamSynchronize(plan->s_d2h);
+        cudaStreamDestroy(plan->s_h2d); cudaStreamDestroy(plan->s_comp); cudaStreamDestroy(plan->s_d2h);
+        cudaEvent_t evs[] = {plan->ev_user, plan->ev_h2d[0], plan->ev_h2d[1], plan->ev_comp[0], plan->ev_comp[1],
+                             plan->ev_d2h[0], plan->ev_d2h[1]};
+        for (cudaEvent_t ev : evs) if (ev) cudaEventDestroy(ev);
+    }
     if (plan->d_cls) cudaFree(plan->d_cls);
     if (plan->d_twz) cudaFree(plan->d_twz);
     for (auto& ev : plan->prof_events) cudaEventDestroy(ev);

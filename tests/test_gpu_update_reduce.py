@@ -160,3 +160,36 @@ def test_paper_thickness_optimisation_on_gpu(hb):
     Href = O.hybrid_layers(n, n, 5, d, d, dz, m[0], None, [4], dft="fft")
     assert abs(Href[0, 2].mean()) < 1e-9
     plan.close()
+
+
+def test_pipelined_host_path_matches_plain_host_path(hb):
+    """hfft_demag_host_async / hfft_host_join: several evaluations in flight over two staging slots give,
+    in call order, exactly the fields of hfft_demag_host; one of them is checked against the oracle."""
+    import torch
+    w = W.small(32, 16, 4, precision="f32", B=2, seed=8)
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, "f32", batch=2)
+    plan.build_tensor()
+    rng = np.random.default_rng(5)
+    ms, want, got = [], [], []
+    for t in range(5):
+        m = rng.normal(size=(2, 3, w.nz, w.ny, w.nx))
+        m /= np.sqrt((m ** 2).sum(axis=1, keepdims=True))
+        ms.append(torch.from_numpy(m).float().pin_memory())
+    for m in ms:
+        want.append(plan.demag_host(m, w.Ms))     # a fresh pinned buffer per call
+    torch.cuda.synchronize()
+    for m in ms:                                     # five calls back to back, nothing synchronised in between
+        got.append(plan.demag_host_async(m, w.Ms))
+    plan.host_join()
+    torch.cuda.synchronize()
+    for a, b in zip(got, want):
+        assert torch.equal(a, b)
+    m3 = ms[3].double().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m3, w.Ms, dft="fft")
+    assert _relerr(got[3].double().numpy(), ref) <= TOL["f32"]
+    # join with nothing outstanding, and errors
+    plan.host_join()
+    with pytest.raises(hb.HfftError) as e:
+        hb.demag_host_async(plan.handle, 0, None, 0)
+    assert e.value.status == hb.EINVAL
+    plan.close()
