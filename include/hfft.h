@@ -106,6 +106,15 @@ hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
  */
 hfft_status hfft_plan_set_dedup(hfft_plan *plan, int mode);
 
+/*
+ * Host-only helper (no device needed): the tensor classes hfft_plan_set_dedup works with.
+ * dz: HOST array of nz thicknesses; cls_out: HOST array of nz*nz ints, cls_out[i*nz+j] = bank slot
+ * of the pair (target i, source j); *n_classes = number of slots; *toeplitz = 1 when the thicknesses
+ * are all equal (slot = |i-j|; the xz, yz entries of the pair carry a minus sign for i < j).
+ * Errors: EINVAL (NULL pointers, nz < 1 or > HFFT_MAX_NZ, non-positive / non-finite dz).
+ */
+hfft_status hfft_tensor_classes(int nz, const double *dz, int *cls_out, int *n_classes, int *toeplitz);
+
 /* Sizes the plan needs; valid after create / set_batch / set_dedup.  Errors: EINVAL. */
 hfft_status hfft_plan_info(const hfft_plan *plan, hfft_info *info);
 

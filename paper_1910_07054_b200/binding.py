@@ -23,7 +23,7 @@ STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
 
 # every symbol include/hfft.h declares
-EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_info", "hfft_plan_set_buffers",
+EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_tensor_classes", "hfft_plan_info", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
@@ -62,6 +62,7 @@ def lib():
                                        ctypes.c_double, ctypes.c_double, dp, ctypes.c_int]
         L.hfft_plan_set_batch.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_dedup.argtypes = [vp, ctypes.c_int]
+        L.hfft_tensor_classes.argtypes = [ctypes.c_int, dp, ip, ip, ip]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.hfft_plan_set_buffers.argtypes = [vp, vp, vp]
         L.hfft_build_tensor.argtypes = [vp, vp]
@@ -119,6 +120,17 @@ def plan_set_batch(plan, batch):
 def plan_set_dedup(plan, mode):
     """0 off, 1 automatic (default), 2 on, 3 z-FFT method (equal thicknesses; Eq.25)."""
     _check(lib().hfft_plan_set_dedup(plan, int(mode)), plan)
+
+
+def tensor_classes(dz):
+    """Host-only: (cls [nz][nz] int array, n_classes, toeplitz) of a stack of thicknesses dz."""
+    dz = np.ascontiguousarray(dz, dtype=np.float64)
+    nz = dz.shape[0]
+    cls = np.zeros(max(nz * nz, 1), dtype=np.int32)
+    n, t = ctypes.c_int(), ctypes.c_int()
+    _check(lib().hfft_tensor_classes(nz, _dptr(dz), cls.ctypes.data_as(ctypes.POINTER(ctypes.c_int)),
+                                     ctypes.byref(n), ctypes.byref(t)))
+    return cls[:nz * nz].reshape(nz, nz), n.value, bool(t.value)
 
 
 def plan_info(plan) -> Info:

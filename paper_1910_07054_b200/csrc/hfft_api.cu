@@ -256,6 +256,19 @@ hfft_status hfft_plan_set_dedup(hfft_plan* plan, int mode) {
     return HFFT_OK;
 }
 
+hfft_status hfft_tensor_classes(int nz, const double* dz, int* cls_out, int* n_classes, int* toeplitz) {
+    if (!dz || !cls_out || !n_classes || !toeplitz || nz < 1 || nz > HFFT_MAX_NZ) return HFFT_EINVAL;
+    for (int k = 0; k < nz; ++k)
+        if (!(dz[k] > 0) || !isfinite(dz[k])) return HFFT_EINVAL;
+    std::vector<int> cls, rep;
+    bool toep = false;
+    pair_classes(nz, dz, cls, rep, toep);
+    for (size_t x = 0; x < cls.size(); ++x) cls_out[x] = cls[x];
+    *n_classes = (int)rep.size();
+    *toeplitz = toep ? 1 : 0;
+    return HFFT_OK;
+}
+
 hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     if (!plan || !info) return HFFT_EINVAL;
     info->nx = plan->nx; info->ny = plan->ny; info->nz = plan->nz; info->batch = plan->batch;
