@@ -189,6 +189,22 @@ def run_reference(args, w):
     print(json.dumps(line))
 
 
+def max_over_ranks(times_ms, device="cpu"):
+    """The timed regions of all ranks, reduced with MAX (the slowest replica sets the job's time).
+    Works on any initialised process group (nccl on the GPUs, gloo in the CPU tests); identity for one process."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(times_ms), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(world, batch, steps, ms_total):
+    """Evaluations per second of the whole job: every rank ran `steps` calls of `batch` states (weak scaling)."""
+    return world * batch * steps / (ms_total * 1e-3)
+
+
 def workload_config(w, l2):
     return {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "batch": w.B, "precision": w.precision,
             "dz_nm": [round(float(v), 6) for v in w.dz[:8]] + (["..."] if w.nz > 8 else []),
@@ -317,15 +333,12 @@ def main():
     clocks = sampler.stop()
 
     assert bool(torch.isfinite(h).all()) and bool(torch.isfinite(h_host).all())
-    t = torch.tensor([ms_total, ms_e2e], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total, ms_e2e = float(t[0]), float(t[1])
+    ms_total, ms_e2e, ms_e2e_serial = max_over_ranks([ms_total, ms_e2e, ms_e2e_serial], device="cuda")
 
     if rank == 0:
         peak, peak_src = measured_peaks()
         ms_step = ms_total / steps
-        value = world * w.B * steps / (ms_total * 1e-3)
+        value = whole_job_value(world, w.B, steps, ms_total)
         coup_ms = float(stage_ms[hb.STAGE_NAMES.index("coupling")])
         achieved = ab["coupling"] / (coup_ms * 1e-3) / 1e9 if coup_ms > 0 else None
         traffic = None
@@ -342,11 +355,11 @@ def main():
                 if flush is None else "L2 flushed (256 MiB memset) before every timed step"),
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
                        "samples": clocks["samples"]},
-            "e2e": {"value": world * w.B * e2e_steps / (ms_e2e * 1e-3), "unit": UNIT,
+            "e2e": {"value": whole_job_value(world, w.B, e2e_steps, ms_e2e), "unit": UNIT,
                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
                     "api": "hfft_demag_host_async + hfft_host_join (per step: pinned host m -> device, 5 kernels, "
                            "device h -> pinned host; copies of neighbouring steps overlap the kernels)",
-                    "serialised_hfft_demag_host": world * w.B * e2e_steps / (ms_e2e_serial * 1e-3)},
+                    "serialised_hfft_demag_host": whole_job_value(world, w.B, e2e_steps, ms_e2e_serial)},
             "gpu_launches": plan.info.launches_per_demag * steps,
             "roofline": {"bound": "hbm", "kernel": "coupling_kernel (S3)", "achieved": achieved, "peak": peak,
                          "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak if achieved else None,
