@@ -239,3 +239,30 @@ def test_zfft_errors(hb):
         r.update_dz(1, 2.0)
     assert e.value.status == hb.EUNSUPPORTED
     r.close()
+
+
+@pytest.mark.parametrize("case", ["plain", "batched", "classes", "toeplitz", "zfft", "plain_f64"])
+def test_repeated_calls_are_bitwise_identical(hb, case):
+    """No kernel of the path uses atomics or an order that depends on scheduling (the fused reductions, off here, are
+    the one exception), so repeated evaluations must agree bit for bit; a shared-memory race in the exchange or
+    staging buffers would show up here (compute-sanitizer is not available on the GPU pool)."""
+    import torch
+    cfg = {
+        "plain": dict(nx=64, ny=128, dz=None, nz=7, B=1, prec="f32", dedup=0),
+        "batched": dict(nx=128, ny=64, dz=None, nz=5, B=4, prec="f32", dedup=0),
+        "classes": dict(nx=64, ny=64, dz=[1.0, 0.5] * 8, nz=16, B=1, prec="f32", dedup=2),
+        "toeplitz": dict(nx=64, ny=64, dz=[0.5] * 40, nz=40, B=2, prec="f32", dedup=2),
+        "zfft": dict(nx=64, ny=64, dz=[0.5] * 40, nz=40, B=2, prec="f32", dedup=3),
+        "plain_f64": dict(nx=32, ny=64, dz=None, nz=6, B=1, prec="f64", dedup=0),
+    }[case]
+    w = W.small(cfg["nx"], cfg["ny"], cfg["nz"], precision=cfg["prec"], B=cfg["B"], seed=17,
+                dz=None if cfg["dz"] is None else np.array(cfg["dz"]))
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, cfg["prec"], batch=cfg["B"], dedup=cfg["dedup"])
+    plan.build_tensor()
+    dt = torch.float32 if cfg["prec"] == "f32" else torch.float64
+    m = torch.from_numpy(w.m_rounded()).to(dt).cuda()
+    first = plan.demag(m, w.Ms).clone()
+    assert bool(torch.isfinite(first).all())
+    for _ in range(25):
+        assert torch.equal(plan.demag(m, w.Ms), first)
+    plan.close()
