@@ -63,13 +63,14 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def algorithmic_bytes(w, n_slots=None):
+def algorithmic_bytes(w, n_slots=None, mirror=False):
     """what the shipped storage must move per hfft_demag call.
-    n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank)."""
+    n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank);
+    mirror: ky-mirror storage, one bank entry per (kx, ky <= ny)."""
     s = 4 if w.precision == "f32" else 8
     n_k = 2 * w.ny * (w.nx + 1)
     planes = 3 * w.nz * w.B
-    bank = 6 * (n_slots if n_slots else w.nz * w.nz) * n_k * s
+    bank = 6 * (n_slots if n_slots else w.nz * w.nz) * ((w.nx + 1) * (w.ny + 1) if mirror else n_k) * s
     spec = planes * n_k * 2 * s            # M^ (= H^)
     xhat = planes * w.ny * (w.nx + 1) * 2 * s
     field = planes * w.ny * w.nx * s
@@ -253,8 +254,9 @@ def main():
     nbytes = m.numel() * m.element_size()
     dedup = int(plan.info.dedup)
     # bank slots per wavevector: nz^2 pairs, tensor classes, or the Lz values of kz in the z-FFT mode
-    slots = int(plan.info.bank_bytes // (6 * plan.info.n_k_padded * (4 if w.precision == "f32" else 8)))
-    ab = algorithmic_bytes(w, slots if dedup else None)
+    mirror = bool(plan.info.mirror)
+    slots = int(plan.info.bank_bytes // (6 * (plan.info.n_k_padded // (2 if mirror else 1)) * (4 if w.precision == "f32" else 8)))
+    ab = algorithmic_bytes(w, slots if dedup else None, mirror)
     # inputs larger than L2?  otherwise flush L2 between steps (and say so)
     flush = None
     if ab["whole"] < 512 << 20:
@@ -386,7 +388,7 @@ def main():
                                 "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
                                 "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
                                 "hbm_gbs": achieved, "traffic": None}
-        line["config"]["bank"] = {"dedup": dedup, "slots_per_k": slots,
+        line["config"]["bank"] = {"dedup": dedup, "ky_mirror": mirror, "slots_per_k": slots,
                                   "bytes": int(plan.info.bank_bytes)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)

@@ -59,14 +59,17 @@ typedef struct {
     int precision;            /* hfft_precision */
     int tile_k;               /* wavevectors per bank tile */
     long long n_k;            /* wavevectors in the Hermitian half spectrum: (nx+1) * 2ny */
-    long long n_k_padded;     /* n_k rounded up to a multiple of tile_k */
-    size_t bank_bytes;        /* spectral tensor bank: 6 * (nz^2 or n_classes) * n_k_padded * sizeof(element) */
+    long long n_k_padded;     /* spectrum slots per plane: n_k (mirror storage: (nx+1) * (2ny+2)) rounded up to a
+                                 multiple of tile_k */
+    size_t bank_bytes;        /* spectral tensor bank: 6 * (nz^2 or n_classes) * n_k_padded * sizeof(element);
+                                 half of that with mirror storage */
     size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging (two slots of m and h) */
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
     int launches_per_demag;   /* kernels hfft_demag enqueues per call */
     int built;                /* 1 once hfft_build_tensor has completed */
     int n_classes;            /* bank slots a deduplicated bank needs: distinct tensors among the nz^2 layer pairs;
                                  nz for equal thicknesses (N_ij and N_ji then differ by the sign of xz, yz only) */
+    int mirror;               /* 1: ky-mirror storage (hfft_plan_set_mirror): half the bank, spectrum rows of 2ny+2 slots */
     int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
                                  shared memory; 3: as 2 with Toeplitz classes (equal thicknesses) */
 } hfft_info;
@@ -105,6 +108,21 @@ hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
  * before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_dedup(hfft_plan *plan, int mode);
+
+/*
+ * ky-mirror storage of the bank.  The in-plane parities of the tensor
+ * components (xx, yy, zz, xz even in Y; xy, yz odd) make their spectra even / odd in
+ * ky, so the wavevectors ky and 2ny - ky share one bank entry (xy, yz with opposite
+ * sign).  The bank then holds ny + 1 entries per kx instead of 2ny -- half the bytes
+ * the HBM-bound coupling stage streams -- and S2 / S4 keep every pair in adjacent
+ * spectrum slots.  on = 1 (default): used wherever the plain streaming coupling kernel
+ * runs with wide tiles (large grids, no deduplication, not the batched register
+ * kernel); on = 0: never; on = 2: also on small grids (wide tiles forced; tests).
+ * info.mirror tells which.  Results are those of the plain
+ * storage (the mirrored entries are equal up to rounding of the fp64 FFT).  Must be
+ * called before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
+ */
+hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
 
 /*
  * Host-only helper (no device needed): the tensor classes hfft_plan_set_dedup works with.

@@ -23,7 +23,8 @@ STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
 
 # every symbol include/hfft.h declares
-EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_tensor_classes", "hfft_plan_info", "hfft_plan_set_buffers",
+EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror",
+           "hfft_tensor_classes", "hfft_plan_info", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
@@ -36,7 +37,7 @@ class Info(ctypes.Structure):
                 ("bank_bytes", ctypes.c_size_t), ("workspace_bytes", ctypes.c_size_t),
                 ("setup_scratch_bytes", ctypes.c_size_t),
                 ("launches_per_demag", ctypes.c_int), ("built", ctypes.c_int),
-                ("n_classes", ctypes.c_int), ("dedup", ctypes.c_int)]
+                ("n_classes", ctypes.c_int), ("mirror", ctypes.c_int), ("dedup", ctypes.c_int)]
 
 
 class HfftError(RuntimeError):
@@ -62,6 +63,7 @@ def lib():
                                        ctypes.c_double, ctypes.c_double, dp, ctypes.c_int]
         L.hfft_plan_set_batch.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_dedup.argtypes = [vp, ctypes.c_int]
+        L.hfft_plan_set_mirror.argtypes = [vp, ctypes.c_int]
         L.hfft_tensor_classes.argtypes = [ctypes.c_int, dp, ip, ip, ip]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.hfft_plan_set_buffers.argtypes = [vp, vp, vp]
@@ -120,6 +122,10 @@ def plan_set_batch(plan, batch):
 def plan_set_dedup(plan, mode):
     """0 off, 1 automatic (default), 2 on, 3 z-FFT method (equal thicknesses; Eq.25)."""
     _check(lib().hfft_plan_set_dedup(plan, int(mode)), plan)
+
+
+def plan_set_mirror(plan, on):
+    _check(lib().hfft_plan_set_mirror(plan, int(on)), plan)
 
 
 def tensor_classes(dz):
@@ -218,7 +224,7 @@ def destroy(plan):
 class Plan:
     """Convenience owner: plan + torch-allocated bank / workspace on the current CUDA device."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None):
+    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None, mirror=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -232,6 +238,8 @@ class Plan:
             plan_set_batch(self.handle, batch)
         if dedup is not None:
             plan_set_dedup(self.handle, dedup)
+        if mirror is not None:
+            plan_set_mirror(self.handle, mirror)
         self.info = plan_info(self.handle)
         self._bank = self._ws = None
         if torch_buffers:

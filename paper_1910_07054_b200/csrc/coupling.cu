@@ -35,6 +35,12 @@ template <> struct BankVec<float, 4> {
         v[0] = t.x; v[1] = t.y; v[2] = t.z; v[3] = t.w;
     }
 };
+template <> struct BankVec<float, 2> {
+    template <bool CACHED> static __device__ __forceinline__ void ld(const float* p, float v[2]) {
+        float2 t = bank_ld<CACHED>(reinterpret_cast<const float2*>(p));
+        v[0] = t.x; v[1] = t.y;
+    }
+};
 template <> struct BankVec<float, 1> {
     template <bool CACHED> static __device__ __forceinline__ void ld(const float* p, float v[1]) { v[0] = bank_ld<CACHED>(p); }
 };
@@ -48,12 +54,18 @@ template <> struct BankVec<double, 1> {
     template <bool CACHED> static __device__ __forceinline__ void ld(const double* p, double v[1]) { v[0] = bank_ld<CACHED>(p); }
 };
 
-template <typename T, int KPT, bool CLS>
+// MIR (mirror layout, fft_kernels.cu ypos): the spectrum slots 2p and 2p + 1 hold ky and its mirror 2ny - ky, which
+// share one bank entry p -- xx, yy, zz, xz are even in ky, xy and yz odd -- so a lane's KPT slots need
+// KPT / 2 bank values per component and the odd slots take -xy, -yz: the bank stream, the only HBM-bound part, halves.
+template <typename T, int KPT, bool CLS, bool MIR>
 __global__ void __launch_bounds__(512)
 coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
                 long long ks, int ncls, const unsigned short* __restrict__ cls, int fold) {
     typedef HFFT_C C;
+    static_assert(!(CLS && MIR) && (!MIR || KPT % 2 == 0), "mirror layout: plain bank, an even number of slots per lane");
     constexpr int TK = 32 * KPT;
+    constexpr int KB = MIR ? KPT / 2 : KPT;               // bank values per lane and component
+    constexpr int TKB = 32 * KB;                          // bank values per tile, pair and component
     constexpr int CHUNK_C = 16 / sizeof(C);               // complex per 16-byte chunk (2 or 1)
     constexpr int CPP = TK / CHUNK_C;                     // chunks per plane row
     constexpr bool SWZ = (KPT * sizeof(C) == 32);         // two 16-byte chunks per lane
@@ -83,17 +95,26 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
             for (int e = 0; e < KPT; ++e) hx[e] = hy[e] = hz[e] = mk<T>((T)0, (T)0);
             // deduplicated bank (CLS): the slot of pair (i, j) is its tensor class; the tile is then small
             // and re-read by every target layer, so it is served from L1 / L2
-            const T* bt = CLS ? bank + tile * ncls * (6LL * TK) + lane * KPT
-                              : bank + ((tile * nz + i) * nz) * (6LL * TK) + lane * KPT;
+            const T* bt = CLS ? bank + tile * ncls * (6LL * TKB) + lane * KB
+                              : bank + ((tile * nz + i) * nz) * (6LL * TKB) + lane * KB;
 #pragma unroll 2
             for (int j = 0; j < nz; ++j) {
-                T a[6][KPT];
+                T ab[6][KB];
                 const int slot = CLS ? (int)cls[i * nz + j] : j;
 #pragma unroll
-                for (int c = 0; c < 6; ++c) BankVec<T, KPT>::template ld<CLS>(bt + (slot * 6 + c) * TK, a[c]);
+                for (int c = 0; c < 6; ++c) BankVec<T, KB>::template ld<CLS>(bt + (slot * 6 + c) * TKB, ab[c]);
                 if (CLS && fold && i < j) {               // folded Toeplitz classes: N_{-d} = N_d with xz, yz negated
 #pragma unroll
-                    for (int e = 0; e < KPT; ++e) { a[4][e] = -a[4][e]; a[5][e] = -a[5][e]; }
+                    for (int e = 0; e < KB; ++e) { ab[4][e] = -ab[4][e]; ab[5][e] = -ab[5][e]; }
+                }
+                T a[6][KPT];                              // per slot; mirror slots (odd) take -xy, -yz
+#pragma unroll
+                for (int e = 0; e < KPT; ++e) {
+                    const int eb = MIR ? e / 2 : e;
+                    const bool neg = MIR && (e & 1);
+                    a[0][e] = ab[0][eb]; a[1][e] = ab[1][eb]; a[2][e] = ab[2][eb]; a[4][e] = ab[4][eb];
+                    a[3][e] = neg ? -ab[3][eb] : ab[3][eb];
+                    a[5][e] = neg ? -ab[5][eb] : ab[5][eb];
                 }
                 C m[3][KPT];
 #pragma unroll
@@ -458,10 +479,10 @@ static cudaError_t launch_coupling_batched(const void* bank, void* spec, int nz,
 
 size_t coupling_smem_bytes(int nz, int tile_k, size_t elem) { return (size_t)3 * nz * tile_k * 2 * elem; }
 
-template <typename T, int KPT, bool CLS>
+template <typename T, int KPT, bool CLS, bool MIR = false>
 static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     typedef HFFT_C C;
-    auto kern = coupling_kernel<T, KPT, CLS>;
+    auto kern = coupling_kernel<T, KPT, CLS, MIR>;
     const size_t smem = coupling_smem_bytes(a.nz, 32 * KPT, sizeof(T));
     const int warps = a.nz < 16 ? a.nz : 16;
     const int threads = warps * 32;
@@ -498,6 +519,7 @@ cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
         if (a.tile_k == 32) return launch_coupling_k<T, 1, true>(a, st);
         return cudaErrorInvalidValue;
     }
+    if (a.mirror) return a.tile_k == 32 * KV ? launch_coupling_k<T, KV, false, true>(a, st) : cudaErrorInvalidValue;
     if (a.tile_k == 32 && coupling_batched_applies(a.nz, a.batch, sizeof(T)))
         return launch_coupling_batched<T>(a.bank, a.spec, a.nz, a.batch, a.n_tiles, a.ks, a.num_sms, st);
     if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, false>(a, st);

@@ -11,7 +11,8 @@
 // Layouts (C = complex of T):
 //   real field      [plane][rows][nx]           plane = (state, component, layer)
 //   X^ (after S1)   [plane][nx+1][rows] C       (kx major, y fastest)
-//   M^ (after S2)   [plane][KS] C, element k = kx * 2ny + ky
+//   M^ (after S2)   [plane][KS] C, element k = kx * 2ny + ky; "mirror" layout: kx * (2ny + 2) + ypos(ky), where
+//                   ypos pairs ky with 2ny - ky in adjacent slots (see ypos below)
 // The z-component planes of M^ hold i*M_z (and H^ holds i*H_z) so that the layer coupling is a
 // real matrix acting on real and imaginary parts alike.
 //
@@ -248,6 +249,14 @@ template <int LOG2N> struct YCfg {
     static constexpr int THREADS = TPR > 128 ? TPR : 128;
 };
 
+// Mirror layout of a spectrum row (hfft_plan_set_mirror): the tensor spectra are even (xx, yy, zz, xz) or
+// odd (xy, yz) in ky, so ky and 2ny - ky can share one bank entry.  A row then has N + 2 slots: ky <= N/2 sits at
+// 2 ky, its mirror N - ky at 2 ky + 1; ky = 0 and ky = N/2 are their own mirrors, their odd slots (1 and N + 1) are
+// dummies that hold zeros (never written by S2, H^ = N^ 0 = 0 written by S3, ignored by S4).
+__device__ __forceinline__ int ypos(int ky, int N, int mirror) {
+    return mirror ? (ky <= N / 2 ? 2 * ky : 2 * (N - ky) + 1) : ky;
+}
+
 // (plane, kx) of a row and whether the plane is a z component (nz_rot layers per component)
 struct RowPos {
     long long plane; int kx; int pl3;
@@ -265,7 +274,7 @@ struct RowPos {
 template <typename T, int LOG2N, bool ZP>
 __global__ void __launch_bounds__(YCfg<LOG2N>::THREADS)
 ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long long nrows, int nxp1, int nz_rot,
-                long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc) {
+                long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc, int mirror) {
     typedef HFFT_C C;
     typedef RowFFT<T, LOG2N, false, ZP, sizeof(T) == 4> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR;
@@ -294,7 +303,7 @@ ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long
         for (int q = 0; q < RL; ++q) v[q] = nv[q];
         const bool cur_live = live;
         const bool rot = pos.is_z(nz_rot);
-        C* dst = spec + pos.plane * ks + (long long)pos.kx * N + j;
+        C* dst = spec + pos.plane * ks + (long long)pos.kx * (mirror ? N + 2 : N);
         row += rpc; zin += zstep;
         live = (it + 1 < nit) && row < nrows;
         if (live) {
@@ -309,7 +318,7 @@ ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long
                 for (int q = 0; q < R; ++q) v[q] = mul_pi(v[q]);
             }
 #pragma unroll
-            for (int q = 0; q < R; ++q) dst[q * TPR] = v[q];
+            for (int q = 0; q < R; ++q) dst[ypos(j + q * TPR, N, mirror)] = v[q];
         }
     }
 }
@@ -317,7 +326,7 @@ ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long
 template <typename T, int LOG2N>
 __global__ void __launch_bounds__(YCfg<LOG2N>::THREADS)
 iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long long nrows, int nxp1, int nz_rot,
-             long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc) {
+             long long ks, const HFFT_C* __restrict__ twt, long long ngroups, int gpc, int mirror) {
     typedef HFFT_C C;
     typedef RowFFT<T, LOG2N, true, false, sizeof(T) == 4> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR;
@@ -334,9 +343,9 @@ iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long lo
     C nv[R];
     bool live = row < nrows;
     if (live) {
-        const C* src = spec + pos.plane * ks + (long long)pos.kx * N + j;
+        const C* src = spec + pos.plane * ks + (long long)pos.kx * (mirror ? N + 2 : N);
 #pragma unroll
-        for (int q = 0; q < R; ++q) nv[q] = src[q * TPR];
+        for (int q = 0; q < R; ++q) nv[q] = src[ypos(j + q * TPR, N, mirror)];
     }
     for (int it = 0; it < nit; ++it) {
         C v[R];
@@ -349,9 +358,9 @@ iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long lo
         live = (it + 1 < nit) && row < nrows;
         if (live) {
             pos.advance(rpc, nxp1, nz_rot);
-            const C* src = spec + pos.plane * ks + (long long)pos.kx * N + j;
+            const C* src = spec + pos.plane * ks + (long long)pos.kx * (mirror ? N + 2 : N);
 #pragma unroll
-            for (int q = 0; q < R; ++q) nv[q] = src[q * TPR];
+            for (int q = 0; q < R; ++q) nv[q] = src[ypos(j + q * TPR, N, mirror)];
         }
         F::run(v, c);
         if (cur_live) {
@@ -494,7 +503,7 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
 
 template <typename T, bool ZP>
 cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                            const void* twt, int num_sms, cudaStream_t st) {
+                            const void* twt, int num_sms, cudaStream_t st, int mirror) {
     typedef HFFT_C C;
     const int N = 1 << log2N;
     const int tpr = fft_tpr(log2N);
@@ -513,7 +522,7 @@ cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
             kern<<<grid, threads, smem, st>>>((const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks, (const C*)twt,
-                                              ngroups, gpc);
+                                              ngroups, gpc, mirror);
             err = cudaGetLastError();
         }
     })
@@ -522,7 +531,7 @@ cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int
 
 template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                         const void* twt, int num_sms, cudaStream_t st) {
+                         const void* twt, int num_sms, cudaStream_t st, int mirror) {
     typedef HFFT_C C;
     const int N = 1 << log2N;
     const int tpr = fft_tpr(log2N);
@@ -541,7 +550,7 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
             kern<<<grid, threads, smem, st>>>((const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks, (const C*)twt,
-                                              ngroups, gpc);
+                                              ngroups, gpc, mirror);
             err = cudaGetLastError();
         }
     })
@@ -554,10 +563,10 @@ template cudaError_t launch_fftx_fwd<double, true>(const double*, void*, int, in
 template cudaError_t launch_fftx_fwd<double, false>(const double*, void*, int, int, int, int, const double*, const void*, const void*, int, cudaStream_t);
 template cudaError_t launch_ifftx<float>(const void*, float*, int, int, int, const void*, const void*, int, const float*, double*, cudaStream_t);
 template cudaError_t launch_ifftx<double>(const void*, double*, int, int, int, const void*, const void*, int, const double*, double*, cudaStream_t);
-template cudaError_t launch_ffty_fwd<float, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
-template cudaError_t launch_ffty_fwd<double, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
-template cudaError_t launch_ffty_fwd<double, false>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
-template cudaError_t launch_iffty<float>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
-template cudaError_t launch_iffty<double>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t);
+template cudaError_t launch_ffty_fwd<float, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t, int);
+template cudaError_t launch_ffty_fwd<double, true>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t, int);
+template cudaError_t launch_ffty_fwd<double, false>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t, int);
+template cudaError_t launch_iffty<float>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t, int);
+template cudaError_t launch_iffty<double>(const void*, void*, int, int, int, int, long long, const void*, int, cudaStream_t, int);
 
 }  // namespace hfft

@@ -41,6 +41,9 @@ struct hfft_plan {
     // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
     int dedup_mode = 1;                              // 0 off, 1 auto, 2 on, 3 z-FFT (Eq.25)
     bool dedup = false, toeplitz = false, class_kernel = false;
+    int mirror_mode = 1;                             // hfft_plan_set_mirror: 0 off, 1 automatic
+    bool mirror = false;                             // spectrum in the mirror layout, half bank (coupling_kernel MIR)
+    long long n_slots = 0;                           // spectrum slots per plane before padding
     bool zfft = false;                               // equal thicknesses: z-convolution by FFT (coupling_zfft.cu)
     int log2lz = 0;
     void* d_twz = nullptr;                           // exp(-2 pi i n / Lz), plan precision
@@ -145,6 +148,7 @@ static cudaError_t upload_thread_twiddles(int log2N, bool f32, void** out) {
 static BuildGeom make_geom(const hfft_plan* p) {
     BuildGeom g{p->nx, p->ny, p->nz, p->log2nx, p->log2ny, p->dx, p->dy, p->dz.data(),
                 p->tile_k, p->n_k, p->n_k_padded, p->prec, p->num_sms};
+    g.mirror = p->mirror;
     if (p->dedup) { g.pair_class = p->pair_class.data(); g.class_rep = p->class_rep.data(); g.n_classes = p->n_classes; }
     return g;
 }
@@ -168,10 +172,18 @@ static void plan_sizes(hfft_plan* p) {
     if (p->tile_k != wide) p->tile_k = 32;
     if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
     if (p->class_kernel || p->zfft) p->tile_k = 32;
-    p->n_tiles = (p->n_k + p->tile_k - 1) / p->tile_k;
+    if (p->mirror_mode == 2 && !p->dedup && !coupling_batched_applies(p->nz, p->batch, e) &&
+        coupling_smem_bytes(p->nz, wide, e) <= 200 * 1024)
+        p->tile_k = wide;                            // forced mirror storage: wide tiles whatever the grid size
+    // ky-mirror storage (the spectra are even or odd in ky): the plain streaming kernel with wide tiles
+    // reads one bank value per pair (ky, 2ny - ky); the spectrum rows then have 2ny + 2 slots (fft_kernels.cu ypos)
+    p->mirror = p->mirror_mode >= 1 && !p->dedup && p->tile_k == wide && p->ny >= 2 &&
+                !coupling_batched_applies(p->nz, p->batch, e);
+    p->n_slots = p->mirror ? (long long)(p->nx + 1) * (2 * p->ny + 2) : p->n_k;
+    p->n_tiles = (p->n_slots + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
     const size_t slots = p->zfft ? ((size_t)1 << p->log2lz) : (p->dedup ? p->n_classes : p->nz * p->nz);
-    p->bank_bytes = (size_t)6 * slots * (size_t)p->n_k_padded * e;
+    p->bank_bytes = (size_t)6 * slots * (size_t)(p->mirror ? p->n_k_padded / 2 : p->n_k_padded) * e;
     const size_t planes = (size_t)3 * p->nz * p->batch;
     auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
     size_t o = 0;
@@ -256,6 +268,15 @@ hfft_status hfft_plan_set_dedup(hfft_plan* plan, int mode) {
     return HFFT_OK;
 }
 
+hfft_status hfft_plan_set_mirror(hfft_plan* plan, int on) {
+    if (!plan) return HFFT_EINVAL;
+    if (on < 0 || on > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_mirror: 0, 1 or 2");
+    if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_mirror: after build / set_buffers");
+    plan->mirror_mode = on;
+    plan_sizes(plan);
+    return HFFT_OK;
+}
+
 hfft_status hfft_tensor_classes(int nz, const double* dz, int* cls_out, int* n_classes, int* toeplitz) {
     if (!dz || !cls_out || !n_classes || !toeplitz || nz < 1 || nz > HFFT_MAX_NZ) return HFFT_EINVAL;
     for (int k = 0; k < nz; ++k)
@@ -280,6 +301,7 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
     info->n_classes = plan->n_classes;
+    info->mirror = plan->mirror ? 1 : 0;
     info->dedup = plan->zfft ? 4 : (plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0);
     return HFFT_OK;
 }
@@ -390,13 +412,14 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
     // the z components are rotated by i on the k side (real form R6) except in the z-FFT mode
     const int nz_rot = p->zfft ? 0 : p->nz;
     STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y,
-                                       p->num_sms, st)))
+                                       p->num_sms, st, p->mirror ? 1 : 0)))
     CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
                     p->dedup ? p->n_classes : p->nz * p->nz, p->dedup ? p->d_cls : nullptr,
                     p->class_kernel, p->toeplitz, p->num_sms};
-    ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz;
+    ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz; ca.mirror = p->mirror;
     STAGE(2, (launch_coupling<T>(ca, st)))
-    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st)))
+    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st,
+                              p->mirror ? 1 : 0)))
     if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
         return fail_cuda(p, "cudaMemsetAsync(sums)", e);
     STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, (const T*)m,
@@ -567,7 +590,9 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     if (p->zfft) return fail(p, HFFT_EUNSUPPORTED, "hfft_read_bank: the bank of the z-FFT mode holds S(k, kz), not N_ij(k)");
     cudaError_t e = cudaDeviceSynchronize();
     if (e != cudaSuccess) return fail_cuda(p, "cudaDeviceSynchronize", e);
-    const int tk = p->tile_k;
+    // bank entries per tile; mirror storage: entry kx * (ny + 1) + t serves ky = t and ky = 2ny - t (xy, yz negated)
+    const int tk = p->mirror ? p->tile_k / 2 : p->tile_k;
+    const long long n_e = p->mirror ? (long long)(p->nx + 1) * (p->ny + 1) : p->n_k;
     // folded Toeplitz classes: the slot holds N_{|i-j|}; xz, yz change sign for i < j
     const double unscale = -4.0 * p->nx * p->ny * ((p->dedup && p->toeplitz && i < j && c >= 4) ? -1.0 : 1.0);
     std::vector<unsigned char> buf((size_t)tk * p->elem);
@@ -578,10 +603,15 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
         e = cudaMemcpy(buf.data(), static_cast<unsigned char*>(p->bank) + off, (size_t)tk * p->elem, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, "cudaMemcpy(bank)", e);
         for (int kk = 0; kk < tk; ++kk) {
-            long long k = t * tk + kk;
-            if (k >= p->n_k) break;
+            const long long en = t * tk + kk;
+            if (en >= n_e) break;
             double v = p->elem == 4 ? (double)reinterpret_cast<float*>(buf.data())[kk] : reinterpret_cast<double*>(buf.data())[kk];
-            out_host[k] = v * unscale;
+            v *= unscale;
+            if (!p->mirror) { out_host[en] = v; continue; }
+            const long long kx = en / (p->ny + 1);
+            const int ty = (int)(en - kx * (p->ny + 1));
+            out_host[kx * 2 * p->ny + ty] = v;
+            if (ty > 0 && ty < p->ny) out_host[kx * 2 * p->ny + (2 * p->ny - ty)] = (c == 3 || c == 5) ? -v : v;
         }
     }
     return HFFT_OK;

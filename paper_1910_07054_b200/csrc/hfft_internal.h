@@ -25,14 +25,15 @@ cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, in
 template <typename T>
 cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw2nx,
                          const void* twt_nx, int num_sms, const T* m, double* sums, cudaStream_t st);
-// forward y: X^ rows [nplanes * (nx+1)][N/2 if ZP else N] -> k side [nplanes][ks], k = kx * N + ky;
+// forward y: X^ rows [nplanes * (nx+1)][N/2 if ZP else N] -> k side [nplanes][ks], k = kx * N + ky
+// (mirror: kx * (N + 2) + ypos(ky), ky and N - ky in adjacent slots; fft_kernels.cu);
 // nz_rot > 0 multiplies the z-component planes by i
 template <typename T, bool ZP>
 cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                            const void* twt_N, int num_sms, cudaStream_t st);
+                            const void* twt_N, int num_sms, cudaStream_t st, int mirror = 0);
 template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
-                         const void* twt_N, int num_sms, cudaStream_t st);
+                         const void* twt_N, int num_sms, cudaStream_t st, int mirror = 0);
 
 // ---- coupling.cu ----
 // H^ = bank * M^ in place on the k side.  bank layout [tile][class][6][tile_k]; class = i*nz+j (cls == nullptr)
@@ -47,6 +48,7 @@ struct CouplingArgs {
     bool toeplitz;                 // equal thicknesses: cls[i*nz+j] == |i - j|, xz / yz negated for i < j
     int num_sms;
     // z-FFT mode (coupling_zfft.cu; Eq.25): bank = S(k, kz) [tile][kz][6][32], Lz = 2^log2lz
+    bool mirror = false;           // spectrum in the mirror layout, one bank value per pair of slots (coupling_kernel MIR)
     bool zfft = false;
     int log2lz = 0;
     const void* twz = nullptr;     // device, exp(-2 pi i n / Lz), plan precision
@@ -78,6 +80,7 @@ struct BuildGeom {
     int num_sms;
     // deduplicated bank: host tables pair -> class [nz*nz], class -> representative pair
     // i*nz+j [n_classes]; pair_class == nullptr: one slot per pair (class = i*nz+j)
+    bool mirror = false;   // bank entry p = kx * (ny + 1) + t, t = 0..ny, serves ky = t and ky = 2ny - t; tile_k / 2 per tile
     const int* pair_class = nullptr;
     const int* class_rep = nullptr;
     int n_classes = 0;

@@ -119,23 +119,31 @@ assemble_kernel(double* __restrict__ R, const double2* __restrict__ psi_lo /* a 
     if (p > 0 && q > 0) dst[(size_t)(H - q) * W + (W - p)] = v * sx * sy;
 }
 
+// bank entry e of a (pair, component): tile_e entries per tile, n_e entries (padded to whole tiles: n_e_padded).
+// Plain layout: e = k.  Mirror layout (fft_kernels.cu ypos): e = kx * (ny + 1) + t, t = 0..ny, taken from k = kx * 2ny + t.
 template <typename T>
 __global__ void __launch_bounds__(256)
 pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, int j0, int ncls,
-            const unsigned short* __restrict__ cls, int tile_k, long long n_k, long long n_k_padded, double scale) {
-    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+            const unsigned short* __restrict__ cls, int tile_e, long long n_k, long long n_e, long long n_e_padded,
+            int mirror_ny, double scale) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int jc = blockIdx.y;          // jl * 6 + c
-    if (k >= n_k_padded) return;
+    if (e >= n_e_padded) return;
     const int jl = jc / 6, c = jc - jl * 6;
     double v = 0.0;
-    if (k < n_k) {
+    if (e < n_e) {
+        long long k = e;
+        if (mirror_ny > 0) {
+            const long long kx = e / (mirror_ny + 1);
+            k = kx * 2 * mirror_ny + (e - kx * (mirror_ny + 1));
+        }
         double2 t = Y[(size_t)jc * n_k + k];
         v = (c < 4 ? t.x : t.y) * scale;
     }
-    const long long tile = k / tile_k;
-    const int kk = (int)(k - tile * tile_k);
+    const long long tile = e / tile_e;
+    const int kk = (int)(e - tile * tile_e);
     const int pr = i * nz + j0 + jl;                       // bank slot = tensor class of the pair
-    bank[((tile * ncls + (cls ? (int)cls[pr] : pr)) * 6 + c) * tile_k + kk] = (T)v;
+    bank[((tile * ncls + (cls ? (int)cls[pr] : pr)) * 6 + c) * tile_e + kk] = (T)v;
 }
 
 struct ScratchLayout {
@@ -316,13 +324,16 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
                                                         g.num_sms, st)));
                 HFFT_CK((launch_ffty_fwd<double, false>(d_X, d_Y, nx, g.log2ny + 1, jn * 6, 0, g.n_k, twt_2ny,
                                                         g.num_sms, st)));
-                dim3 gridp((unsigned)((g.n_k_padded + 255) / 256), jn * 6);
+                const int tile_e = g.mirror ? g.tile_k / 2 : g.tile_k;
+                const long long n_e = g.mirror ? (long long)(nx + 1) * (ny + 1) : g.n_k;
+                const long long n_e_padded = g.mirror ? g.n_k_padded / 2 : g.n_k_padded;
+                dim3 gridp((unsigned)((n_e_padded + 255) / 256), jn * 6);
                 if (g.prec == HFFT_F32)
-                    pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, ncls, d_cls, g.tile_k, g.n_k,
-                                                              g.n_k_padded, scale);
+                    pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, ncls, d_cls, tile_e, g.n_k, n_e,
+                                                              n_e_padded, g.mirror ? ny : 0, scale);
                 else
-                    pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, ncls, d_cls, g.tile_k,
-                                                               g.n_k, g.n_k_padded, scale);
+                    pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, ncls, d_cls, tile_e, g.n_k,
+                                                               n_e, n_e_padded, g.mirror ? ny : 0, scale);
                 HFFT_CK(cudaGetLastError());
             }
     }

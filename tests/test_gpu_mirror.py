@@ -1,0 +1,107 @@
+"""ky-mirror storage of the bank (hfft_plan_set_mirror) against the oracle through the C ABI.  -m gpu.
+
+The spectra of xx, yy, zz, xz are even in ky, those of xy, yz odd, so ky and 2ny - ky share one bank entry; S2 / S4
+keep each pair in adjacent spectrum slots.  mode 2 forces the storage on small grids (ragged tiles, tiny ny)."""
+import numpy as np
+import pytest
+
+import oracle as O
+from paper_1910_07054_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+TOL = {"f32": 2e-6, "f64": 1e-12}
+
+
+@pytest.fixture(scope="module")
+def hb():
+    import torch
+    from paper_1910_07054_b200 import binding
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    binding.lib()
+    return binding
+
+
+def _relerr(a, b):
+    return float(np.abs(a - b).max() / np.abs(b).max())
+
+
+SHAPES = [(16, 16, 3, 1), (8, 2, 2, 1), (2, 4, 1, 1), (32, 8, 5, 2), (4, 64, 4, 1), (64, 32, 17, 1), (128, 16, 2, 3)]
+
+
+@pytest.mark.parametrize("nx,ny,nz,B", SHAPES)
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_mirror_storage_vs_oracle(hb, nx, ny, nz, B, prec):
+    import torch
+    w = W.small(nx, ny, nz, precision=prec, B=B, seed=900 + nx + 3 * ny + 7 * nz)
+    m = w.m_rounded()
+    plan = hb.Plan(nx, ny, nz, w.dx, w.dy, w.dz, prec, batch=B, dedup=0, mirror=2)
+    plan.build_tensor()
+    info = hb.plan_info(plan.handle)
+    batched_kernel = B > 1 and 6 * nz * (4 if prec == "f32" else 8) <= 384      # register-bank kernel keeps its layout
+    assert info.mirror == (0 if batched_kernel else 1)
+    if info.mirror:
+        s = 4 if prec == "f32" else 8
+        assert info.n_k_padded >= (nx + 1) * (2 * ny + 2)
+        assert info.bank_bytes == 6 * nz * nz * (info.n_k_padded // 2) * s
+    dt = torch.float32 if prec == "f32" else torch.float64
+    md = torch.from_numpy(m).to(dt).cuda()
+    for _ in range(2):                                   # second call: the dummy slots still hold zeros
+        H = plan.demag(md, w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    if nx * ny * nz <= 2048:
+        ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, w.dz, m[0], w.Ms)          # the definition, Eq.18
+        assert _relerr(H[0], ref0) <= TOL[prec]
+    plan.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_mirror_bank_reads_back_like_the_plain_bank(hb, prec):
+    """hfft_read_bank reconstructs every wavevector from the half bank (signs of xy, yz for ky > ny included)."""
+    w = W.small(16, 8, 3, precision=prec, seed=12)
+    a = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec, dedup=0, mirror=0)
+    b = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec, dedup=0, mirror=2)
+    a.build_tensor()
+    b.build_tensor()
+    assert hb.plan_info(a.handle).mirror == 0 and hb.plan_info(b.handle).mirror == 1
+    worst = 0.0
+    for i in range(3):
+        for j in range(3):
+            for c in range(6):
+                x, y = hb.read_bank(a.handle, i, j, c), hb.read_bank(b.handle, i, j, c)
+                worst = max(worst, np.abs(x - y).max() / max(np.abs(x).max(), 1e-30))
+    assert worst <= (1e-6 if prec == "f32" else 1e-12)    # mirrored entries agree to the rounding of the fp64 FFT
+    a.close()
+    b.close()
+
+
+def test_mirror_with_update_dz_and_reductions(hb):
+    import torch
+    w = W.small(32, 16, 4, precision="f64", seed=33)
+    dz2 = w.dz.copy()
+    dz2[1] = 2.25
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, "f64", dedup=0, mirror=2)
+    plan.build_tensor()
+    plan.update_dz(1, 2.25)
+    sums = plan.set_reduction(True)
+    m = w.m_rounded()
+    H = plan.demag(torch.from_numpy(m).cuda(), w.Ms).cpu().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, dz2, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f64"]
+    assert np.abs(sums.cpu().numpy()[..., 0] - ref.sum(axis=(-1, -2))).max() <= 1e-10 * np.abs(ref).max() * w.nx * w.ny
+    plan.close()
+
+
+def test_mirror_errors_and_automatic_mode(hb):
+    p = hb.Plan(16, 16, 3, 1.0, 1.0, np.array([1.0, 2.0, 0.5]), "f32")
+    assert hb.plan_info(p.handle).mirror == 0            # small grid: narrow tiles, plain storage
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_set_mirror(p.handle, 3)
+    assert e.value.status == hb.EINVAL
+    with pytest.raises(hb.HfftError) as e:
+        hb.plan_set_mirror(p.handle, 0)
+    assert e.value.status == hb.ESTATE
+    p.close()
+    q = hb.Plan(256, 256, 4, 2.0, 2.0, np.array([1.0, 2.0, 0.5, 0.7]), "f32", torch_buffers=False)
+    assert hb.plan_info(q.handle).mirror == 1            # large grid: automatic
+    q.close()
