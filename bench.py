@@ -43,6 +43,8 @@ def parse_args():
     ap.add_argument("--config", default="4", help="BASELINE.json config 1..5, '2f64', '4eq'")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mirror", type=int, default=None, help="hfft_plan_set_mirror mode (default: the library's, 1)")
+    ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
     return ap.parse_args()
 
 
@@ -239,7 +241,7 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B)
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B, dedup=args.dedup, mirror=args.mirror)
     t0 = time.perf_counter()
     plan.build_tensor()
     torch.cuda.synchronize()

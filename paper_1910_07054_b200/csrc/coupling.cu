@@ -95,14 +95,27 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
             for (int e = 0; e < KPT; ++e) hx[e] = hy[e] = hz[e] = mk<T>((T)0, (T)0);
             // deduplicated bank (CLS): the slot of pair (i, j) is its tensor class; the tile is then small
             // and re-read by every target layer, so it is served from L1 / L2
+            // MIR: the 6 KB values of a lane are stored as three vectors of 2 KB (component pairs (xx,yy), (zz,xy),
+            // (xz,yz) x KB entries: [pair][lane][2][KB]), so that the half-width bank still moves in 16-byte loads --
+            // with 8-byte loads the same bytes in flight need twice the outstanding requests and HBM idles (ncu)
             const T* bt = CLS ? bank + tile * ncls * (6LL * TKB) + lane * KB
-                              : bank + ((tile * nz + i) * nz) * (6LL * TKB) + lane * KB;
-#pragma unroll 2
+                              : bank + ((tile * nz + i) * nz) * (6LL * TKB) + lane * (MIR ? 2 * KB : KB);
+#pragma unroll (MIR ? 4 : 2)
             for (int j = 0; j < nz; ++j) {
                 T ab[6][KB];
                 const int slot = CLS ? (int)cls[i * nz + j] : j;
+                if constexpr (MIR) {
 #pragma unroll
-                for (int c = 0; c < 6; ++c) BankVec<T, KB>::template ld<CLS>(bt + (slot * 6 + c) * TKB, ab[c]);
+                    for (int cp = 0; cp < 3; ++cp) {
+                        T v2[2 * KB];
+                        BankVec<T, 2 * KB>::template ld<false>(bt + (slot * 6 + 2 * cp) * TKB, v2);
+#pragma unroll
+                        for (int e = 0; e < KB; ++e) { ab[2 * cp][e] = v2[e]; ab[2 * cp + 1][e] = v2[KB + e]; }
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) BankVec<T, KB>::template ld<CLS>(bt + (slot * 6 + c) * TKB, ab[c]);
+                }
                 if (CLS && fold && i < j) {               // folded Toeplitz classes: N_{-d} = N_d with xz, yz negated
 #pragma unroll
                     for (int e = 0; e < KB; ++e) { ab[4][e] = -ab[4][e]; ab[5][e] = -ab[5][e]; }
@@ -133,6 +146,9 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                             m[c][0] = row[s0 * CHUNK_C];
                             m[c][1 % KPT] = row[s1 * CHUNK_C];
                         }
+                    } else if (KPT == 2 && sizeof(T) == 4) {
+                        const float4 u = *reinterpret_cast<const float4*>(row + lane * 2);   // one 16-byte chunk per lane
+                        m[c][0] = mk<T>(u.x, u.y); m[c][1 % KPT] = mk<T>(u.z, u.w);
                     } else {
 #pragma unroll
                         for (int e = 0; e < KPT; ++e) m[c][e] = row[lane * KPT + e];
@@ -140,9 +156,15 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                 }
 #pragma unroll
                 for (int e = 0; e < KPT; ++e) {
+                    if (MIR) {      // twice the arithmetic per bank byte: packed FFMA2 (HFFT_MIR_PACKED experiment)
+                        hx[e] = caxpy(a[0][e], m[0][e], hx[e]); hx[e] = caxpy(a[3][e], m[1][e], hx[e]); hx[e] = caxpy(a[4][e], m[2][e], hx[e]);
+                        hy[e] = caxpy(a[3][e], m[0][e], hy[e]); hy[e] = caxpy(a[1][e], m[1][e], hy[e]); hy[e] = caxpy(a[5][e], m[2][e], hy[e]);
+                        hz[e] = caxpy(a[2][e], m[2][e], hz[e]); hz[e] = caxpy(-a[4][e], m[0][e], hz[e]); hz[e] = caxpy(-a[5][e], m[1][e], hz[e]);
+                    } else {
                     hx[e] = caxpy_s(a[0][e], m[0][e], hx[e]); hx[e] = caxpy_s(a[3][e], m[1][e], hx[e]); hx[e] = caxpy_s(a[4][e], m[2][e], hx[e]);
                     hy[e] = caxpy_s(a[3][e], m[0][e], hy[e]); hy[e] = caxpy_s(a[1][e], m[1][e], hy[e]); hy[e] = caxpy_s(a[5][e], m[2][e], hy[e]);
                     hz[e] = caxpy_s(a[2][e], m[2][e], hz[e]); hz[e] = caxpy_s(-a[4][e], m[0][e], hz[e]); hz[e] = caxpy_s(-a[5][e], m[1][e], hz[e]);
+                    }
                 }
             }
             C* ox = sp + (long long)(0 * nz + i) * ks + lane * KPT;
@@ -155,6 +177,10 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                 reinterpret_cast<float4*>(oy)[1] = make_float4(hy[2 % KPT].x, hy[2 % KPT].y, hy[3 % KPT].x, hy[3 % KPT].y);
                 reinterpret_cast<float4*>(oz)[0] = make_float4(hz[0].x, hz[0].y, hz[1 % KPT].x, hz[1 % KPT].y);
                 reinterpret_cast<float4*>(oz)[1] = make_float4(hz[2 % KPT].x, hz[2 % KPT].y, hz[3 % KPT].x, hz[3 % KPT].y);
+            } else if (KPT == 2 && sizeof(T) == 4) {
+                reinterpret_cast<float4*>(ox)[0] = make_float4(hx[0].x, hx[0].y, hx[1 % KPT].x, hx[1 % KPT].y);
+                reinterpret_cast<float4*>(oy)[0] = make_float4(hy[0].x, hy[0].y, hy[1 % KPT].x, hy[1 % KPT].y);
+                reinterpret_cast<float4*>(oz)[0] = make_float4(hz[0].x, hz[0].y, hz[1 % KPT].x, hz[1 % KPT].y);
             } else {
 #pragma unroll
                 for (int e = 0; e < KPT; ++e) { ox[e] = hx[e]; oy[e] = hy[e]; oz[e] = hz[e]; }
@@ -519,7 +545,7 @@ cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
         if (a.tile_k == 32) return launch_coupling_k<T, 1, true>(a, st);
         return cudaErrorInvalidValue;
     }
-    if (a.mirror) return a.tile_k == 32 * KV ? launch_coupling_k<T, KV, false, true>(a, st) : cudaErrorInvalidValue;
+    if (a.mirror) return a.tile_k == 64 ? launch_coupling_k<T, 2, false, true>(a, st) : cudaErrorInvalidValue;
     if (a.tile_k == 32 && coupling_batched_applies(a.nz, a.batch, sizeof(T)))
         return launch_coupling_batched<T>(a.bank, a.spec, a.nz, a.batch, a.n_tiles, a.ks, a.num_sms, st);
     if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, false>(a, st);

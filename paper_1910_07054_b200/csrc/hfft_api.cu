@@ -167,18 +167,20 @@ static void plan_sizes(hfft_plan* p) {
                       coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
     // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
     const int wide = 32 * (int)(16 / e);
-    p->tile_k = (p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148)) ? wide : 32;
+    const bool big = p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148);
+    p->tile_k = big ? wide : 32;
     while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
     if (p->tile_k != wide) p->tile_k = 32;
     if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
     if (p->class_kernel || p->zfft) p->tile_k = 32;
-    if (p->mirror_mode == 2 && !p->dedup && !coupling_batched_applies(p->nz, p->batch, e) &&
-        coupling_smem_bytes(p->nz, wide, e) <= 200 * 1024)
-        p->tile_k = wide;                            // forced mirror storage: wide tiles whatever the grid size
-    // ky-mirror storage (the spectra are even or odd in ky): the plain streaming kernel with wide tiles
-    // reads one bank value per pair (ky, 2ny - ky); the spectrum rows then have 2ny + 2 slots (fft_kernels.cu ypos)
-    p->mirror = p->mirror_mode >= 1 && !p->dedup && p->tile_k == wide && p->ny >= 2 &&
-                !coupling_batched_applies(p->nz, p->batch, e);
+    // ky-mirror storage (the spectra are even or odd in ky): where the plain streaming kernel would run
+    // with wide tiles (mode 2: on any grid) it reads one bank value per pair (ky, 2ny - ky); the spectrum rows then
+    // have 2ny + 2 slots (fft_kernels.cu ypos).  Tiles of 64 slots = 32 bank entries, one per lane, in both
+    // precisions: measured faster than 128-slot tiles in fp32 (B200, C4: 1.11 vs 1.28 ms, C3: 0.084 vs 0.098 ms --
+    // two or more CTAs with their M^ tiles share an SM).
+    p->mirror = p->mirror_mode >= 1 && !p->dedup && (big || p->mirror_mode == 2) && p->ny >= 2 &&
+                !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
+    if (p->mirror) p->tile_k = 64;
     p->n_slots = p->mirror ? (long long)(p->nx + 1) * (2 * p->ny + 2) : p->n_k;
     p->n_tiles = (p->n_slots + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
@@ -599,13 +601,19 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     for (long long t = 0; t < p->n_tiles; ++t) {
         const size_t ncls = p->dedup ? p->n_classes : (size_t)p->nz * p->nz;
         const size_t slot = p->dedup ? p->pair_class[(size_t)i * p->nz + j] : (size_t)i * p->nz + j;
-        const size_t off = (((size_t)t * ncls + slot) * 6 + c) * tk * p->elem;
-        e = cudaMemcpy(buf.data(), static_cast<unsigned char*>(p->bank) + off, (size_t)tk * p->elem, cudaMemcpyDeviceToHost);
+        // plain: [c][tk]; mirror: [component pair][lane][2][KB] (tensor_build.cu pack_kernel) -- read the pair's block
+        const size_t blk = ((size_t)t * ncls + slot) * 6 * tk;
+        const size_t off = (blk + (p->mirror ? (size_t)(c >> 1) * 2 * tk : (size_t)c * tk)) * p->elem;
+        const size_t cnt = p->mirror ? 2 * (size_t)tk : (size_t)tk;
+        if (buf.size() < cnt * p->elem) buf.resize(cnt * p->elem);
+        e = cudaMemcpy(buf.data(), static_cast<unsigned char*>(p->bank) + off, cnt * p->elem, cudaMemcpyDeviceToHost);
         if (e != cudaSuccess) return fail_cuda(p, "cudaMemcpy(bank)", e);
+        const int KB = tk / 32;
         for (int kk = 0; kk < tk; ++kk) {
             const long long en = t * tk + kk;
             if (en >= n_e) break;
-            double v = p->elem == 4 ? (double)reinterpret_cast<float*>(buf.data())[kk] : reinterpret_cast<double*>(buf.data())[kk];
+            const int idx = p->mirror ? ((kk / KB) * 2 + (c & 1)) * KB + kk % KB : kk;
+            double v = p->elem == 4 ? (double)reinterpret_cast<float*>(buf.data())[idx] : reinterpret_cast<double*>(buf.data())[idx];
             v *= unscale;
             if (!p->mirror) { out_host[en] = v; continue; }
             const long long kx = en / (p->ny + 1);

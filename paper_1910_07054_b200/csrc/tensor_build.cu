@@ -143,7 +143,14 @@ pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, 
     const long long tile = e / tile_e;
     const int kk = (int)(e - tile * tile_e);
     const int pr = i * nz + j0 + jl;                       // bank slot = tensor class of the pair
-    bank[((tile * ncls + (cls ? (int)cls[pr] : pr)) * 6 + c) * tile_e + kk] = (T)v;
+    const long long blk = (tile * ncls + (cls ? (int)cls[pr] : pr)) * 6LL * tile_e;
+    if (mirror_ny > 0) {
+        // [component pair][lane][2][KB]: a lane's two components of a pair are one 16-byte vector (coupling.cu MIR)
+        const int KB = tile_e / 32, lane = kk / KB, kl = kk - lane * KB;
+        bank[blk + (((c >> 1) * 32 + lane) * 2 + (c & 1)) * KB + kl] = (T)v;
+    } else {
+        bank[blk + (long long)c * tile_e + kk] = (T)v;
+    }
 }
 
 struct ScratchLayout {
