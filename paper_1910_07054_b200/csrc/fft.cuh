@@ -225,14 +225,14 @@ struct RowFFT {
         const C* twp;                              // twt + j
         unsigned st[NSTAGES][R];                   // st[s][u]: store base of butterfly u after stage s
         unsigned ld;                               // load base: element j of the row
-        int bar;                                   // named barrier of the row (TPR > 32)
+        int bar, barn;                             // named barrier of the row (TPR > 32) and its thread count
     };
 
     // the row synchronises among its own threads only: within one warp when TPR <= 32, else on
     // the row's own named barrier (bar.sync id, TPR), so rows of a CTA never wait for each other
     static __device__ __forceinline__ void sync(const Ctx& c) {
         if (TPR <= 32) __syncwarp();
-        else asm volatile("bar.sync %0, %1;" ::"r"(c.bar), "n"(TPR) : "memory");
+        else asm volatile("bar.sync %0, %1;" ::"r"(c.bar), "r"(c.barn) : "memory");
     }
 
     template <int LNS, int SIDX>
@@ -254,9 +254,11 @@ struct RowFFT {
     // rowaddr: shared-space address of the row's buffer pair (ROW_BYTES aligned); rx < min(16, N)
     // is XOR-ed into every element index of the row (lets a caller read the rows "transposed",
     // lanes along rows, without bank conflicts); twt: per-thread twiddle table.
+    // rpb: rows that share one named barrier (there are 15 of them: a CTA with 16 multi-warp rows pairs them up)
     static __device__ __forceinline__ void init(Ctx& c, int r, unsigned rowaddr, int j, int rx,
-                                                const C* __restrict__ twt) {
-        c.bar = r + 1;
+                                                const C* __restrict__ twt, int rpb = 1) {
+        c.bar = r / rpb + 1;
+        c.barn = TPR * rpb;
         c.ld = rowaddr ^ ((unsigned)(swz(j) ^ rx) << SH);
         c.twp = twt + j;
         if constexpr (REGTW) {
