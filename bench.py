@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--config", default="4", help="BASELINE.json config 1..5, '2f64', '4eq'")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep-nz", action="store_true",
+                    help="layer-count scaling at 256 x 256 fp32 (the experiment of PAPER.md:189-203, Fig.3/4): one JSON "
+                         "line per (nz, method) instead of the bench line")
     ap.add_argument("--mirror", type=int, default=None, help="hfft_plan_set_mirror mode (default: the library's, 1)")
     ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
     return ap.parse_args()
@@ -208,6 +211,52 @@ def whole_job_value(world, batch, steps, ms_total):
     return world * batch * steps / (ms_total * 1e-3)
 
 
+def sweep_nz():
+    """evaluation time against the number of layers at nx = ny = 256, non-equidistant hybrid method
+    (fit a x^2 + b x + c) against the equidistant methods (a x log x + b).  Synthetic: dz log-uniform in [0.3, 3] nm
+    (hybrid) or 1 nm (equidistant), random unit vectors, fp32, mean of 20-50 back-to-back calls, best of 3."""
+    import torch
+    from paper_1910_07054_b200 import binding as hb
+    nx = ny = 256
+    for nz in [2, 4, 8, 16, 32, 64, 96, 128]:
+        m = torch.randn(1, 3, nz, ny, nx, device="cuda", dtype=torch.float32)
+        m /= m.norm(dim=1, keepdim=True)
+        h = torch.empty_like(m)
+        dz_var = np.exp(np.random.default_rng(SEED_SWEEP + nz).uniform(np.log(0.3), np.log(3.0), size=nz))
+        for name, dz, kw in [("hybrid (ky-mirror bank)", dz_var, dict(dedup=0)),
+                             ("hybrid (plain bank)", dz_var, dict(dedup=0, mirror=0)),
+                             ("equidistant, Toeplitz classes", np.full(nz, 1.0), dict(dedup=2)),
+                             ("equidistant, z-FFT (Eq.25)", np.full(nz, 1.0), dict(dedup=3))]:
+            if kw.get("mirror") == 0 and nz > 64:
+                continue                                     # plain bank of 29 / 52 GB: not needed for the comparison
+            plan = hb.Plan(nx, ny, nz, 2.0, 2.0, dz, "f32", **kw)
+            t0 = time.perf_counter()
+            plan.build_tensor()
+            torch.cuda.synchronize()
+            setup = time.perf_counter() - t0
+            info = hb.plan_info(plan.handle)
+            for _ in range(5):
+                plan.demag(m, 8e5, h)
+            n = 50 if nz <= 32 else 20
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            best = 1e30
+            for _ in range(3):
+                e0.record()
+                for _ in range(n):
+                    plan.demag(m, 8e5, h)
+                e1.record()
+                torch.cuda.synchronize()
+                best = min(best, e0.elapsed_time(e1) / n)
+            print(json.dumps({"nz": nz, "method": name, "ms_per_eval": best, "setup_s": setup,
+                              "bank_GB": info.bank_bytes / 1e9, "dedup": info.dedup, "mirror": info.mirror}), flush=True)
+            plan.close()
+            del plan
+            torch.cuda.empty_cache()
+
+
+SEED_SWEEP = 191007054
+
+
 def workload_config(w, l2):
     return {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "batch": w.B, "precision": w.precision,
             "dz_nm": [round(float(v), 6) for v in w.dz[:8]] + (["..."] if w.nz > 8 else []),
@@ -216,6 +265,9 @@ def workload_config(w, l2):
 
 def main():
     args = parse_args()
+    if args.sweep_nz:
+        sweep_nz()
+        return
     w = get_workload(args.config)
     if args.impl == "reference":
         run_reference(args, w)

@@ -105,3 +105,18 @@ def test_mirror_errors_and_automatic_mode(hb):
     q = hb.Plan(256, 256, 4, 2.0, 2.0, np.array([1.0, 2.0, 0.5, 0.7]), "f32", torch_buffers=False)
     assert hb.plan_info(q.handle).mirror == 1            # large grid: automatic
     q.close()
+
+
+def test_mirror_many_layers_one_cta_per_sm(hb):
+    """fp32, nz = 80: the M^ tile (120 KB) leaves room for one CTA per SM, which then runs 32 warps."""
+    import torch
+    nz = 80
+    w = W.small(8, 8, nz, precision="f32", seed=80)
+    m = w.m_rounded()
+    plan = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, w.dz, "f32", dedup=0, mirror=2)
+    plan.build_tensor()
+    assert hb.plan_info(plan.handle).mirror == 1
+    H = plan.demag(torch.from_numpy(m).float().cuda(), w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f32"]
+    plan.close()
