@@ -47,6 +47,7 @@ def parse_args():
                     help="layer-count scaling at 256 x 256 fp32 (the experiment of PAPER.md:189-203, Fig.3/4): one JSON "
                          "line per (nz, method) instead of the bench line")
     ap.add_argument("--mirror", type=int, default=None, help="hfft_plan_set_mirror mode (default: the library's, 1)")
+    ap.add_argument("--recip", type=int, default=None, help="hfft_plan_set_recip (default: the library's)")
     ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
     return ap.parse_args()
 
@@ -293,7 +294,8 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
-    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B, dedup=args.dedup, mirror=args.mirror)
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B, dedup=args.dedup, mirror=args.mirror,
+                   recip=args.recip)
     t0 = time.perf_counter()
     plan.build_tensor()
     torch.cuda.synchronize()
@@ -310,7 +312,7 @@ def main():
     # bank slots per wavevector: nz^2 pairs, tensor classes, or the Lz values of kz in the z-FFT mode
     mirror = bool(plan.info.mirror)
     slots = int(plan.info.bank_bytes // (6 * (plan.info.n_k_padded // (2 if mirror else 1)) * (4 if w.precision == "f32" else 8)))
-    ab = algorithmic_bytes(w, slots if dedup else None, mirror)
+    ab = algorithmic_bytes(w, slots if (dedup or int(plan.info.mirror) == 2) else None, mirror)
     # inputs larger than L2?  otherwise flush L2 between steps (and say so)
     flush = None
     if ab["whole"] < 512 << 20:
@@ -442,7 +444,7 @@ def main():
                                 "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
                                 "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
                                 "hbm_gbs": achieved, "traffic": None}
-        line["config"]["bank"] = {"dedup": dedup, "ky_mirror": mirror, "slots_per_k": slots,
+        line["config"]["bank"] = {"dedup": dedup, "ky_mirror": mirror, "reciprocity": int(plan.info.mirror) == 2, "slots_per_k": slots,
                                   "bytes": int(plan.info.bank_bytes)}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)

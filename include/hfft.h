@@ -69,7 +69,8 @@ typedef struct {
     int built;                /* 1 once hfft_build_tensor has completed */
     int n_classes;            /* bank slots a deduplicated bank needs: distinct tensors among the nz^2 layer pairs;
                                  nz for equal thicknesses (N_ij and N_ji then differ by the sign of xz, yz only) */
-    int mirror;               /* 1: ky-mirror storage (hfft_plan_set_mirror): half the bank, spectrum rows of 2ny+2 slots */
+    int mirror;               /* 1: ky-mirror storage (hfft_plan_set_mirror): half the bank, spectrum rows of 2ny+2 slots;
+                                 2: with reciprocity storage on top (hfft_plan_set_recip): a quarter of the bank */
     int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
                                  shared memory; 3: as 2 with Toeplitz classes (equal thicknesses) */
 } hfft_info;
@@ -123,6 +124,19 @@ hfft_status hfft_plan_set_dedup(hfft_plan *plan, int mode);
  * called before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
+
+/*
+ * Reciprocity storage of the bank, on top of the ky-mirror storage.
+ * dz_i N_ij(X,Y) = dz_j N_ji(-X,-Y): in the real form of the coupling, S_ij := dz_i R_ij
+ * satisfies S_ji = S_ij^T, so the bank keeps S_pq for p <= q only -- nz(nz+1)/2 instead
+ * of nz^2 layer pairs, half the bytes again -- the pair (q, p) uses the transpose (xz, yz
+ * negated) and H_i is multiplied by 1/dz_i at the end.  Every entry is then needed by two
+ * target layers; the kernel orders its reads so that the second one is served by L2.
+ * on = 1 takes effect wherever the mirror storage is active (info.mirror == 2 then);
+ * default 0.  hfft_update_dz rebuilds the whole bank in this mode.  Must be called before
+ * hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
+ */
+hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
 
 /*
  * Host-only helper (no device needed): the tensor classes hfft_plan_set_dedup works with.

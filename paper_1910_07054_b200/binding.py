@@ -23,7 +23,7 @@ STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
 
 # every symbol include/hfft.h declares
-EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror",
+EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror", "hfft_plan_set_recip",
            "hfft_tensor_classes", "hfft_plan_info", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
@@ -64,6 +64,7 @@ def lib():
         L.hfft_plan_set_batch.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_dedup.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_mirror.argtypes = [vp, ctypes.c_int]
+        L.hfft_plan_set_recip.argtypes = [vp, ctypes.c_int]
         L.hfft_tensor_classes.argtypes = [ctypes.c_int, dp, ip, ip, ip]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.hfft_plan_set_buffers.argtypes = [vp, vp, vp]
@@ -126,6 +127,10 @@ def plan_set_dedup(plan, mode):
 
 def plan_set_mirror(plan, on):
     _check(lib().hfft_plan_set_mirror(plan, int(on)), plan)
+
+
+def plan_set_recip(plan, on):
+    _check(lib().hfft_plan_set_recip(plan, int(on)), plan)
 
 
 def tensor_classes(dz):
@@ -224,7 +229,7 @@ def destroy(plan):
 class Plan:
     """Convenience owner: plan + torch-allocated bank / workspace on the current CUDA device."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None, mirror=None):
+    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None, mirror=None, recip=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -240,6 +245,8 @@ class Plan:
             plan_set_dedup(self.handle, dedup)
         if mirror is not None:
             plan_set_mirror(self.handle, mirror)
+        if recip is not None:
+            plan_set_recip(self.handle, recip)
         self.info = plan_info(self.handle)
         self._bank = self._ws = None
         if torch_buffers:

@@ -60,9 +60,12 @@ template <> struct BankVec<double, 1> {
 template <typename T, int KPT, bool CLS, bool MIR>
 __global__ void __launch_bounds__(MIR && sizeof(T) == 4 ? 1024 : 512)
 coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, int batch, long long n_tiles,
-                long long ks, int ncls, const unsigned short* __restrict__ cls, int fold) {
+                long long ks, int ncls, const unsigned short* __restrict__ cls, int fold, const T* __restrict__ inv_dz) {
     typedef HFFT_C C;
-    static_assert(!(CLS && MIR) && (!MIR || KPT % 2 == 0), "mirror layout: plain bank, an even number of slots per lane");
+    static_assert(!MIR || KPT % 2 == 0, "mirror layout: an even number of slots per lane");
+    // CLS && MIR = reciprocity storage (hfft_plan_set_recip): slot(i, j) = slot(j, i); the bank holds S_pq = dz_p R_pq
+    // for p <= q only, the pair (q, p) uses its transpose (xz, yz negated), and H_i is scaled by 1 / dz_i at the end.
+    constexpr bool RECIP = CLS && MIR;
     constexpr int TK = 32 * KPT;
     constexpr int KB = MIR ? KPT / 2 : KPT;               // bank values per lane and component
     constexpr int TKB = 32 * KB;                          // bank values per tile, pair and component
@@ -98,17 +101,26 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
             // MIR: the 6 KB values of a lane are stored as three vectors of 2 KB (component pairs (xx,yy), (zz,xy),
             // (xz,yz) x KB entries: [pair][lane][2][KB]), so that the half-width bank still moves in 16-byte loads --
             // with 8-byte loads the same bytes in flight need twice the outstanding requests and HBM idles (ncu)
-            const T* bt = CLS ? bank + tile * ncls * (6LL * TKB) + lane * KB
+            const T* bt = CLS ? bank + tile * ncls * (6LL * TKB) + lane * (MIR ? 2 * KB : KB)
                               : bank + ((tile * nz + i) * nz) * (6LL * TKB) + lane * (MIR ? 2 * KB : KB);
+            // RECIP: the source layers are visited by increasing |j - i| (j = i, i+1, i-1, i+2, ...): the warps of
+            // targets p and q then read the shared entry (p, q) at about the same time, so that the second read is
+            // served by L2 and HBM delivers every entry once
+            const int rmin = i < nz - 1 - i ? i : nz - 1 - i;
 #pragma unroll (MIR ? 4 : 2)
-            for (int j = 0; j < nz; ++j) {
+            for (int t = 0; t < nz; ++t) {
+                int j = t;
+                if (RECIP) {
+                    const int d = (t + 1) >> 1;
+                    j = t <= 2 * rmin ? ((t & 1) ? i + d : i - d) : (i <= nz - 1 - i ? t : nz - 1 - t);
+                }
                 T ab[6][KB];
                 const int slot = CLS ? (int)cls[i * nz + j] : j;
                 if constexpr (MIR) {
 #pragma unroll
                     for (int cp = 0; cp < 3; ++cp) {
                         T v2[2 * KB];
-                        BankVec<T, 2 * KB>::template ld<false>(bt + (slot * 6 + 2 * cp) * TKB, v2);
+                        BankVec<T, 2 * KB>::template ld<CLS>(bt + (slot * 6 + 2 * cp) * TKB, v2);
 #pragma unroll
                         for (int e = 0; e < KB; ++e) { ab[2 * cp][e] = v2[e]; ab[2 * cp + 1][e] = v2[KB + e]; }
                     }
@@ -116,7 +128,9 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
 #pragma unroll
                     for (int c = 0; c < 6; ++c) BankVec<T, KB>::template ld<CLS>(bt + (slot * 6 + c) * TKB, ab[c]);
                 }
-                if (CLS && fold && i < j) {               // folded Toeplitz classes: N_{-d} = N_d with xz, yz negated
+                // folded Toeplitz classes (fold 1): N_{-d} = N_d with xz, yz negated; reciprocity (fold 2): the pair
+                // (i, j), i > j, is the transpose of the stored (j, i)
+                if (CLS && ((fold == 1 && i < j) || (fold == 2 && i > j))) {
 #pragma unroll
                     for (int e = 0; e < KB; ++e) { ab[4][e] = -ab[4][e]; ab[5][e] = -ab[5][e]; }
                 }
@@ -166,6 +180,11 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
                     hz[e] = caxpy_s(a[2][e], m[2][e], hz[e]); hz[e] = caxpy_s(-a[4][e], m[0][e], hz[e]); hz[e] = caxpy_s(-a[5][e], m[1][e], hz[e]);
                     }
                 }
+            }
+            if (RECIP) {
+                const T sc = inv_dz[i];
+#pragma unroll
+                for (int e = 0; e < KPT; ++e) { hx[e] = cscale(sc, hx[e]); hy[e] = cscale(sc, hy[e]); hz[e] = cscale(sc, hz[e]); }
             }
             C* ox = sp + (long long)(0 * nz + i) * ks + lane * KPT;
             C* oy = sp + (long long)(1 * nz + i) * ks + lane * KPT;
@@ -534,7 +553,7 @@ static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     long long grid = (long long)a.num_sms * occ_blocks;
     if (grid > items) grid = items;
     kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.nz, a.batch, a.n_tiles, a.ks,
-                                                a.n_classes, a.cls, a.toeplitz ? 1 : 0);
+                                                a.n_classes, a.cls, a.recip ? 2 : (a.toeplitz ? 1 : 0), (const T*)a.inv_dz);
     return cudaGetLastError();
 }
 
@@ -542,6 +561,7 @@ template <typename T>
 cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
     constexpr int KV = 16 / sizeof(T);
     if (a.zfft) return launch_coupling_zfft<T>(a, st);
+    if (a.mirror && a.recip) return a.tile_k == 64 ? launch_coupling_k<T, 2, true, true>(a, st) : cudaErrorInvalidValue;
     if (a.cls) {
         if (a.class_kernel) return a.tile_k == 32 ? launch_coupling_class<T>(a, st) : cudaErrorInvalidValue;
         if (a.tile_k == 32 * KV) return launch_coupling_k<T, KV, true>(a, st);

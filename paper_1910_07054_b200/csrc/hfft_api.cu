@@ -41,6 +41,10 @@ struct hfft_plan {
     // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
     int dedup_mode = 1;                              // 0 off, 1 auto, 2 on, 3 z-FFT (Eq.25)
     bool dedup = false, toeplitz = false, class_kernel = false;
+    int recip_mode = 0;                              // hfft_plan_set_recip
+    bool recip = false;                              // bank holds dz_p R_pq for p <= q only (with the mirror storage)
+    std::vector<int> recip_cls, recip_rep;           // pair -> slot of the unordered pair; slot -> p*nz+q (p <= q)
+    void* d_invdz = nullptr;                         // 1 / dz_i, plan precision (recip)
     int mirror_mode = 1;                             // hfft_plan_set_mirror: 0 off, 1 automatic
     bool mirror = false;                             // spectrum in the mirror layout, half bank (coupling_kernel MIR)
     long long n_slots = 0;                           // spectrum slots per plane before padding
@@ -150,7 +154,22 @@ static BuildGeom make_geom(const hfft_plan* p) {
                 p->tile_k, p->n_k, p->n_k_padded, p->prec, p->num_sms};
     g.mirror = p->mirror;
     if (p->dedup) { g.pair_class = p->pair_class.data(); g.class_rep = p->class_rep.data(); g.n_classes = p->n_classes; }
+    if (p->recip) {
+        g.pair_class = p->recip_cls.data(); g.class_rep = p->recip_rep.data(); g.n_classes = (int)p->recip_rep.size();
+        g.recip = true;
+    }
     return g;
+}
+
+// 1 / dz_i in the plan precision (reciprocity storage: H_i = (1 / dz_i) sum_j S_ij M_j)
+static cudaError_t upload_inv_dz(hfft_plan* p) {
+    cudaError_t e;
+    if (!p->d_invdz && (e = cudaMalloc(&p->d_invdz, p->nz * p->elem)) != cudaSuccess) return e;
+    std::vector<float> f(p->nz);
+    std::vector<double> d(p->nz);
+    for (int k = 0; k < p->nz; ++k) { d[k] = 1.0 / p->dz[k]; f[k] = (float)d[k]; }
+    return cudaMemcpy(p->d_invdz, p->elem == 4 ? (const void*)f.data() : (const void*)d.data(), p->nz * p->elem,
+                      cudaMemcpyHostToDevice);
 }
 
 static void plan_sizes(hfft_plan* p) {
@@ -181,10 +200,22 @@ static void plan_sizes(hfft_plan* p) {
     p->mirror = p->mirror_mode >= 1 && !p->dedup && (big || p->mirror_mode == 2) && p->ny >= 2 &&
                 !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
     if (p->mirror) p->tile_k = 64;
+    p->recip = p->mirror && p->recip_mode == 1 && p->nz >= 2 && p->nz * (p->nz + 1) / 2 <= 65535;
+    if (p->recip && p->recip_rep.empty()) {
+        const int nz = p->nz;
+        p->recip_cls.assign((size_t)nz * nz, 0);
+        for (int a = 0; a < nz; ++a)
+            for (int b = a; b < nz; ++b) {
+                const int slot = (int)p->recip_rep.size();
+                p->recip_rep.push_back(a * nz + b);
+                p->recip_cls[(size_t)a * nz + b] = p->recip_cls[(size_t)b * nz + a] = slot;
+            }
+    }
     p->n_slots = p->mirror ? (long long)(p->nx + 1) * (2 * p->ny + 2) : p->n_k;
     p->n_tiles = (p->n_slots + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
-    const size_t slots = p->zfft ? ((size_t)1 << p->log2lz) : (p->dedup ? p->n_classes : p->nz * p->nz);
+    const size_t slots = p->zfft ? ((size_t)1 << p->log2lz)
+                         : (p->recip ? (size_t)p->nz * (p->nz + 1) / 2 : (p->dedup ? p->n_classes : p->nz * p->nz));
     p->bank_bytes = (size_t)6 * slots * (size_t)(p->mirror ? p->n_k_padded / 2 : p->n_k_padded) * e;
     const size_t planes = (size_t)3 * p->nz * p->batch;
     auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
@@ -279,6 +310,15 @@ hfft_status hfft_plan_set_mirror(hfft_plan* plan, int on) {
     return HFFT_OK;
 }
 
+hfft_status hfft_plan_set_recip(hfft_plan* plan, int on) {
+    if (!plan) return HFFT_EINVAL;
+    if (on != 0 && on != 1) return fail(plan, HFFT_EINVAL, "hfft_plan_set_recip: 0 or 1");
+    if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_recip: after build / set_buffers");
+    plan->recip_mode = on;
+    plan_sizes(plan);
+    return HFFT_OK;
+}
+
 hfft_status hfft_tensor_classes(int nz, const double* dz, int* cls_out, int* n_classes, int* toeplitz) {
     if (!dz || !cls_out || !n_classes || !toeplitz || nz < 1 || nz > HFFT_MAX_NZ) return HFFT_EINVAL;
     for (int k = 0; k < nz; ++k)
@@ -303,7 +343,7 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
     info->n_classes = plan->n_classes;
-    info->mirror = plan->mirror ? 1 : 0;
+    info->mirror = plan->mirror ? (plan->recip ? 2 : 1) : 0;
     info->dedup = plan->zfft ? 4 : (plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0);
     return HFFT_OK;
 }
@@ -347,8 +387,10 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
             plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
         }
     }
-    if (plan->dedup && !plan->d_cls) {
-        std::vector<unsigned short> c16(plan->pair_class.begin(), plan->pair_class.end());
+    if (plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) return fail_cuda(plan, "1/dz table", e);
+    if ((plan->dedup || plan->recip) && !plan->d_cls) {
+        const std::vector<int>& tab = plan->recip ? plan->recip_cls : plan->pair_class;
+        std::vector<unsigned short> c16(tab.begin(), tab.end());
         if ((e = cudaMalloc(&plan->d_cls, c16.size() * sizeof(unsigned short))) != cudaSuccess)
             return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(class table): ") + cudaGetErrorString(e));
         if ((e = cudaMemcpy(plan->d_cls, c16.data(), c16.size() * sizeof(unsigned short), cudaMemcpyHostToDevice)) != cudaSuccess)
@@ -416,8 +458,9 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
     STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y,
                                        p->num_sms, st, p->mirror ? 1 : 0)))
     CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
-                    p->dedup ? p->n_classes : p->nz * p->nz, p->dedup ? p->d_cls : nullptr,
-                    p->class_kernel, p->toeplitz, p->num_sms};
+                    p->recip ? (int)p->recip_rep.size() : (p->dedup ? p->n_classes : p->nz * p->nz),
+                    (p->dedup || p->recip) ? p->d_cls : nullptr, p->class_kernel, p->toeplitz, p->num_sms};
+    ca.recip = p->recip; ca.inv_dz = p->d_invdz;
     ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz; ca.mirror = p->mirror;
     STAGE(2, (launch_coupling<T>(ca, st)))
     STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st,
@@ -469,7 +512,10 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
     if ((e = cudaMalloc(&scratch, build_scratch_bytes(g))) != cudaSuccess)
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
     std::string msg;
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, k, st, msg);
+    // reciprocity storage: every stored S_pq = dz_p R_pq of a changed pair is rebuilt from its representative (the
+    // class tables select them), which here means the whole bank; and the 1 / dz table changes
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, plan->recip ? -1 : k, st, msg);
+    if (e == cudaSuccess && plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) msg = "1/dz table";
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
     if (e != cudaSuccess) { plan->built = false; return fail(plan, HFFT_ECUDA, "hfft_update_dz: " + msg); }
@@ -596,11 +642,14 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     const int tk = p->mirror ? p->tile_k / 2 : p->tile_k;
     const long long n_e = p->mirror ? (long long)(p->nx + 1) * (p->ny + 1) : p->n_k;
     // folded Toeplitz classes: the slot holds N_{|i-j|}; xz, yz change sign for i < j
-    const double unscale = -4.0 * p->nx * p->ny * ((p->dedup && p->toeplitz && i < j && c >= 4) ? -1.0 : 1.0);
+    // reciprocity storage: the slot of the unordered pair holds dz_p R_pq (p <= q); (q, p) is its transpose
+    const double unscale = -4.0 * p->nx * p->ny * ((p->dedup && p->toeplitz && i < j && c >= 4) ? -1.0 : 1.0) *
+                           (p->recip ? ((i > j && c >= 4) ? -1.0 : 1.0) / p->dz[i] : 1.0);
     std::vector<unsigned char> buf((size_t)tk * p->elem);
     for (long long t = 0; t < p->n_tiles; ++t) {
-        const size_t ncls = p->dedup ? p->n_classes : (size_t)p->nz * p->nz;
-        const size_t slot = p->dedup ? p->pair_class[(size_t)i * p->nz + j] : (size_t)i * p->nz + j;
+        const size_t ncls = p->recip ? p->recip_rep.size() : (p->dedup ? p->n_classes : (size_t)p->nz * p->nz);
+        const size_t slot = p->recip ? p->recip_cls[(size_t)i * p->nz + j]
+                                     : (p->dedup ? p->pair_class[(size_t)i * p->nz + j] : (size_t)i * p->nz + j);
         // plain: [c][tk]; mirror: [component pair][lane][2][KB] (tensor_build.cu pack_kernel) -- read the pair's block
         const size_t blk = ((size_t)t * ncls + slot) * 6 * tk;
         const size_t off = (blk + (p->mirror ? (size_t)(c >> 1) * 2 * tk : (size_t)c * tk)) * p->elem;
@@ -640,6 +689,7 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     }
     if (plan->d_cls) cudaFree(plan->d_cls);
     if (plan->d_twz) cudaFree(plan->d_twz);
+    if (plan->d_invdz) cudaFree(plan->d_invdz);
     for (auto& ev : plan->prof_events) cudaEventDestroy(ev);
     delete plan;
     return HFFT_OK;

@@ -48,6 +48,8 @@ struct CouplingArgs {
     bool toeplitz;                 // equal thicknesses: cls[i*nz+j] == |i - j|, xz / yz negated for i < j
     int num_sms;
     // z-FFT mode (coupling_zfft.cu; Eq.25): bank = S(k, kz) [tile][kz][6][32], Lz = 2^log2lz
+    bool recip = false;            // reciprocity storage: cls = slot of the unordered pair, bank = dz_p R_pq (p <= q)
+    const void* inv_dz = nullptr;  // device, [nz] plan precision (recip)
     bool mirror = false;           // spectrum in the mirror layout, one bank value per pair of slots (coupling_kernel MIR)
     bool zfft = false;
     int log2lz = 0;
@@ -81,6 +83,7 @@ struct BuildGeom {
     // deduplicated bank: host tables pair -> class [nz*nz], class -> representative pair
     // i*nz+j [n_classes]; pair_class == nullptr: one slot per pair (class = i*nz+j)
     bool mirror = false;   // bank entry p = kx * (ny + 1) + t, t = 0..ny, serves ky = t and ky = 2ny - t; tile_k / 2 per tile
+    bool recip = false;    // bank value of the representative pair (p, q), p <= q, is multiplied by dz_p
     const int* pair_class = nullptr;
     const int* class_rep = nullptr;
     int n_classes = 0;

@@ -320,6 +320,8 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
         // -1 / (4 pi dx dy dz_i) in double-double
         dd tau = dd_mul_d(two_prod(g.dx, g.dy), g.dz[i]);
         dd coef = dd_neg(dd_div(inv4pi, tau));
+        // reciprocity storage keeps S_ij = dz_i R_ij (then S_ji = S_ij^T): the factor goes into the packing
+        const double pscale = g.recip ? scale * g.dz[i] : scale;
         for (const auto& run : runs[i])
             for (int j0 = run.first; j0 <= run.second; j0 += L.jc) {
                 const int jn = (run.second + 1 - j0 < L.jc) ? run.second + 1 - j0 : L.jc;
@@ -337,10 +339,10 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
                 dim3 gridp((unsigned)((n_e_padded + 255) / 256), jn * 6);
                 if (g.prec == HFFT_F32)
                     pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, ncls, d_cls, tile_e, g.n_k, n_e,
-                                                              n_e_padded, g.mirror ? ny : 0, scale);
+                                                              n_e_padded, g.mirror ? ny : 0, pscale);
                 else
                     pack_kernel<double><<<gridp, 256, 0, st>>>((double*)bank, d_Y, nz, i, j0, ncls, d_cls, tile_e, g.n_k,
-                                                               n_e, n_e_padded, g.mirror ? ny : 0, scale);
+                                                               n_e, n_e_padded, g.mirror ? ny : 0, pscale);
                 HFFT_CK(cudaGetLastError());
             }
     }

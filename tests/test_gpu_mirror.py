@@ -120,3 +120,65 @@ def test_mirror_many_layers_one_cta_per_sm(hb):
     ref = O.hybrid_field(w.nx, w.ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
     assert _relerr(H, ref) <= TOL["f32"]
     plan.close()
+
+
+# ---- reciprocity storage on top (hfft_plan_set_recip): S_pq = dz_p R_pq kept for p <= q only ----
+@pytest.mark.parametrize("nx,ny,nz,B", [(16, 16, 3, 1), (8, 2, 2, 1), (32, 8, 5, 2), (4, 64, 4, 1), (64, 32, 17, 1),
+                                        (16, 8, 33, 1), (8, 8, 80, 1)])
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_reciprocity_storage_vs_oracle(hb, nx, ny, nz, B, prec):
+    import torch
+    w = W.small(nx, ny, nz, precision=prec, B=B, seed=1900 + nx + 3 * ny + 7 * nz)
+    m = w.m_rounded()
+    plan = hb.Plan(nx, ny, nz, w.dx, w.dy, w.dz, prec, batch=B, dedup=0, mirror=2, recip=1)
+    plan.build_tensor()
+    info = hb.plan_info(plan.handle)
+    batched_kernel = B > 1 and 6 * nz * (4 if prec == "f32" else 8) <= 384
+    too_many_layers = 3 * nz * 64 * (8 if prec == "f32" else 16) > 200 * 1024      # the M^ tile must fit shared memory
+    assert info.mirror == (0 if batched_kernel or too_many_layers else 2)
+    if info.mirror == 2:
+        assert info.bank_bytes == 6 * (nz * (nz + 1) // 2) * (info.n_k_padded // 2) * (4 if prec == "f32" else 8)
+    dt = torch.float32 if prec == "f32" else torch.float64
+    H = plan.demag(torch.from_numpy(m).to(dt).cuda(), w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    if nx * ny * nz <= 2048:
+        ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, w.dz, m[0], w.Ms)
+        assert _relerr(H[0], ref0) <= TOL[prec]
+    plan.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_reciprocity_bank_reads_back_like_the_plain_bank(hb, prec):
+    """Every ordered pair, read through the half bank (transpose sign and 1/dz_i included), equals the plain entry:
+    this is reciprocity R3, dz_i N_ij(X, Y) = dz_j N_ji(-X, -Y), checked on the device-built tensors."""
+    w = W.small(16, 8, 4, precision=prec, seed=14)
+    a = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec, dedup=0, mirror=0)
+    b = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec, dedup=0, mirror=2, recip=1)
+    a.build_tensor()
+    b.build_tensor()
+    assert hb.plan_info(b.handle).mirror == 2
+    worst = 0.0
+    for i in range(4):
+        for j in range(4):
+            for c in range(6):
+                x, y = hb.read_bank(a.handle, i, j, c), hb.read_bank(b.handle, i, j, c)
+                worst = max(worst, np.abs(x - y).max() / max(np.abs(x).max(), 1e-30))
+    assert worst <= (2e-6 if prec == "f32" else 1e-12)
+    a.close()
+    b.close()
+
+
+def test_reciprocity_with_update_dz(hb):
+    import torch
+    w = W.small(32, 16, 4, precision="f64", seed=35)
+    dz2 = w.dz.copy()
+    dz2[2] = 0.9
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, "f64", dedup=0, mirror=2, recip=1)
+    plan.build_tensor()
+    plan.update_dz(2, 0.9)
+    m = w.m_rounded()
+    H = plan.demag(torch.from_numpy(m).cuda(), w.Ms).cpu().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, dz2, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f64"]
+    plan.close()
