@@ -18,6 +18,13 @@
 // and the whole [i][j][6] stream of a tile is contiguous in memory.  M^ of all layers for the
 // tile sits in shared memory (cp.async, 16-byte chunks, XOR-swizzled against bank conflicts);
 // H^ overwrites M^ in place (each tile is read completely before it is written).
+//
+// Storage variants of the same sum (each with its own kernel or template flag below):
+//   mirror   (MIR)      ky and 2ny - ky share one bank entry: [tile][i][j][3 pairs][32 lanes][2], half the stream
+//   recip    (CLS+MIR)  S_pq = dz_p R_pq for p <= q only, (q, p) by transposition: a quarter of the memory
+//   classes  (CLS, coupling_class_kernel)  one slot per distinct (dz_i, dz_j, Z_ij); Toeplitz window for equal dz
+//   batched  (coupling_batched_kernel)     B states per call, the bank of a tile held in registers
+//   z-FFT    (coupling_zfft.cu)            equal dz: the z-convolution by FFT, Eq.25
 #include "hfft_internal.h"
 #include "fft.cuh"
 
