@@ -362,6 +362,28 @@ def main():
             torch.cuda.synchronize()
             ms_total += ev0.elapsed_time(ev1)
     barrier()
+    # ---- small (launch-bound) configs only: the same step replayed from a CUDA graph (hfft_demag is capturable) ----
+    ms_graph = None
+    if flush is not None:
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            plan.demag(m, Ms, h)
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph, stream=side):
+            plan.demag(m, Ms, h)
+        ms_graph = 0.0
+        for _ in range(steps):
+            flush.zero_()
+            ev0.record()
+            graph.replay()
+            ev1.record()
+            torch.cuda.synchronize()
+            ms_graph += ev0.elapsed_time(ev1)
+        ms_graph /= steps
+        del graph
+    barrier()
     # ---- timed region 2: same steps with per-stage CUDA events (hfft_profile_*) ----
     hb.profile_enable(plan.handle, True)
     stage_ms = np.zeros(hb.NUM_STAGES)
@@ -444,6 +466,9 @@ def main():
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
             "setup_s": setup_s,
         }
+        if ms_graph is not None:
+            line["cuda_graph"] = {"ms_per_step": ms_graph, "evals_per_s": w.B / (ms_graph * 1e-3),
+                                  "note": "the same hfft_demag captured once and replayed (L2 flushed before every replay)"}
         if dedup == 4:
             line["roofline"]["kernel"] = "coupling_zfft_kernel (S3, z-convolution by FFT, PAPER.md:182 Eq.25)"
         if dedup in (2, 3):

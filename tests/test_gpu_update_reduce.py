@@ -193,3 +193,36 @@ def test_pipelined_host_path_matches_plain_host_path(hb):
         hb.demag_host_async(plan.handle, 0, None, 0)
     assert e.value.status == hb.EINVAL
     plan.close()
+
+
+@pytest.mark.parametrize("kw", [dict(), dict(dedup=0, mirror=2), dict(dedup=3)])
+def test_demag_is_capturable_in_a_cuda_graph(hb, kw):
+    """hfft.h: hfft_demag only enqueues kernels (no synchronisation, no allocation) -- so a CUDA graph can capture it;
+    replays with new data in the captured buffers give the fields of direct calls."""
+    import torch
+    dz = np.full(16, 0.5) if kw.get("dedup") == 3 else None
+    w = W.small(32, 16, 16 if dz is not None else 4, precision="f32", seed=61, dz=dz)
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, "f32", **kw)
+    plan.build_tensor()
+    m = torch.from_numpy(w.m_rounded()).float().cuda()
+    h = torch.empty_like(m)
+    side = torch.cuda.Stream()
+    side.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(side):
+        plan.demag(m, w.Ms, h)                       # warm-up outside the capture (function attributes, occupancy caches)
+    torch.cuda.synchronize()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=side):
+        plan.demag(m, w.Ms, h)
+    rng = np.random.default_rng(3)
+    for _ in range(3):
+        mm = rng.normal(size=tuple(m.shape))
+        mm /= np.sqrt((mm ** 2).sum(axis=1, keepdims=True))
+        m.copy_(torch.from_numpy(mm).float())
+        g.replay()
+        torch.cuda.synchronize()
+        got = h.clone()
+        want = plan.demag(m, w.Ms)
+        torch.cuda.synchronize()
+        assert torch.equal(got, want)
+    plan.close()
