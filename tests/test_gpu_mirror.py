@@ -182,3 +182,19 @@ def test_reciprocity_with_update_dz(hb):
     ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, dz2, m, w.Ms, dft="fft")
     assert _relerr(H, ref) <= TOL["f64"]
     plan.close()
+
+
+@pytest.mark.parametrize("prec,nx,ny", [("f64", 128, 128), ("f32", 256, 128), ("f32", 128, 256)])
+def test_mirror_automatic_mode_on_mid_size_grids(hb, prec, nx, ny):
+    """Grids large enough for the automatic choice (no forcing): the mirror storage is what a default plan uses."""
+    import torch
+    w = W.small(nx, ny, 3, precision=prec, seed=5 + nx)
+    m = w.m_rounded()
+    plan = hb.Plan(nx, ny, 3, w.dx, w.dy, w.dz, prec)
+    plan.build_tensor()
+    assert hb.plan_info(plan.handle).mirror == 1 and hb.plan_info(plan.handle).tile_k == 64
+    dt = torch.float32 if prec == "f32" else torch.float64
+    H = plan.demag(torch.from_numpy(m).to(dt).cuda(), w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(nx, ny, 3, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL[prec]
+    plan.close()
