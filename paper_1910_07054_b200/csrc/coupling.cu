@@ -85,6 +85,7 @@ coupling_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, int nz, i
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, nwarps = blockDim.x >> 5;
     const int np = 3 * nz;
     const long long n_items = n_tiles * batch;
+    pdl_wait();                                           // M^ comes from the previous kernel (S2)
 
     for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
         const long long tile = item / batch;
@@ -239,6 +240,7 @@ coupling_batched_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, i
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* sm = reinterpret_cast<C*>(smem_raw);               // [STAGES][NP][TK]
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    pdl_wait();                                           // M^ comes from the previous kernel (S2)
 
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         C* sp = spec + tile * TK;
@@ -349,6 +351,7 @@ coupling_class_kernel(const T* __restrict__ bank, HFFT_C* __restrict__ spec, con
     if (!TOEP) {
         for (int x = tid; x < nz * nz; x += blockDim.x) scls[x] = cls[x];
     }
+    pdl_wait();                                           // M^ comes from the previous kernel (S2)
     for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
         {
             const T* src = bank + tile * ncls * (6LL * TK);
@@ -454,9 +457,8 @@ static cudaError_t launch_coupling_class_t(const CouplingArgs& a, cudaStream_t s
     if (nb < 1) return cudaErrorInvalidConfiguration;
     long long grid = (long long)a.num_sms * nb;
     if (grid > a.n_tiles) grid = a.n_tiles;
-    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.cls, a.nz, a.n_classes, a.batch,
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(threads), smem, st, (const T*)a.bank, (C*)a.spec, a.cls, a.nz, a.n_classes, a.batch,
                                                 a.n_tiles, a.ks);
-    return cudaGetLastError();
 }
 
 template <typename T>
@@ -505,8 +507,7 @@ static cudaError_t launch_coupling_batched_nz(const void* bank, void* spec, int 
     }
     long long grid = (long long)num_sms * occ_blocks;
     if (grid > n_tiles) grid = n_tiles;
-    kern<<<(unsigned)grid, THREADS, smem, st>>>((const T*)bank, (C*)spec, batch, n_tiles, ks);
-    return cudaGetLastError();
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(THREADS), smem, st, (const T*)bank, (C*)spec, batch, n_tiles, ks);
 }
 
 template <typename T>
@@ -559,9 +560,8 @@ static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     long long items = a.n_tiles * a.batch;
     long long grid = (long long)a.num_sms * occ_blocks;
     if (grid > items) grid = items;
-    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, a.nz, a.batch, a.n_tiles, a.ks,
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(threads), smem, st, (const T*)a.bank, (C*)a.spec, a.nz, a.batch, a.n_tiles, a.ks,
                                                 a.n_classes, a.cls, a.recip ? 2 : (a.toeplitz ? 1 : 0), (const T*)a.inv_dz);
-    return cudaGetLastError();
 }
 
 template <typename T>

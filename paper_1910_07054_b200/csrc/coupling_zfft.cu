@@ -119,7 +119,8 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
         }
         cp_async_commit();
     };
-    fetch_bank(blockIdx.x);
+    fetch_bank(blockIdx.x);                                 // the S tile is constant data: it may fly before the wait
+    pdl_wait();                                             // M^ comes from the previous kernel (S2)
     __syncthreads();
 
     for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
@@ -282,9 +283,8 @@ static cudaError_t launch_zfft_l(const CouplingArgs& a, cudaStream_t st) {
     const long long items = a.n_tiles * a.batch;
     long long grid = (long long)a.num_sms * occ;
     if (grid > items) grid = items;
-    kern<<<(unsigned)grid, threads, smem, st>>>((const T*)a.bank, (C*)a.spec, (const C*)a.twz, a.nz, a.batch, a.n_tiles,
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(threads), smem, st, (const T*)a.bank, (C*)a.spec, (const C*)a.twz, a.nz, a.batch, a.n_tiles,
                                                 a.ks);
-    return cudaGetLastError();
 }
 
 template <typename T>

@@ -23,6 +23,10 @@
 
 namespace hfft {
 
+// programmatic dependent launch: wait until the preceding kernel of the stream has completed and its writes are
+// visible (no-op when the kernel was not launched as a dependent)
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 template <typename T> struct cplx_of;
 template <> struct cplx_of<float> { typedef float2 type; };
 template <> struct cplx_of<double> { typedef double2 type; };

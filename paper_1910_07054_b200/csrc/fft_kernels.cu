@@ -85,6 +85,7 @@ fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb,
     const C* zin = reinterpret_cast<const C*>(in) + (blk * rb + r) * (ZP ? N / 2 : N) + j;
     const long long zstep = (long long)rb * (ZP ? N / 2 : N);
     C v[R];
+    pdl_wait();                                              // the previous kernel of the stream may still write `in`
 #pragma unroll
     for (int q = 0; q < RL; ++q) v[q] = zin[q * TPR];
 
@@ -181,6 +182,7 @@ ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, i
         }
         cp_async_commit();
     };
+    pdl_wait();                                              // X^ comes from the previous kernel (S4)
     fetch(plane, y0);
 
     for (int it0 = 0; it0 < nit; ++it0) {
@@ -295,6 +297,7 @@ ffty_fwd_kernel(const HFFT_C* __restrict__ xhat, HFFT_C* __restrict__ spec, long
     const long long zstep = (long long)rpc * (ZP ? N / 2 : N);
     C nv[RL];
     bool live = row < nrows;
+    pdl_wait();                                              // X^ comes from the previous kernel (S1)
     if (live) {
 #pragma unroll
         for (int q = 0; q < RL; ++q) nv[q] = zin[q * TPR];
@@ -344,6 +347,7 @@ iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long lo
     RowPos pos; pos.set(row < nrows ? row : nrows - 1, nxp1, nz_rot);
     C nv[R];
     bool live = row < nrows;
+    pdl_wait();                                              // H^ comes from the previous kernel (S3)
     if (live) {
         const C* src = spec + pos.plane * ks + (long long)pos.kx * (mirror ? N + 2 : N);
 #pragma unroll
@@ -454,9 +458,8 @@ cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, in
         if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int bpc;
             chunk_grid(nblocks, num_sms, occ, grid, bpc);
-            kern<<<grid, threads, smem, st>>>(in, (C*)xhat, log2rb, rows_per_plane, nz > 0 ? nz : 1, use_ms, ms,
+            err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, in, (C*)xhat, log2rb, rows_per_plane, nz > 0 ? nz : 1, use_ms, ms,
                                               (const C*)tw, (const C*)twt, nblocks, bpc);
-            err = cudaGetLastError();
         }
     })
     return err;
@@ -481,9 +484,8 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
             if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
                 unsigned grid; int bpc;
                 chunk_grid(nblocks, num_sms, occ, grid, bpc);
-                kern<<<grid, threads, smem, st>>>((const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
+                err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
                                                   (const C*)twt, nblocks, bpc, m, sums);
-                err = cudaGetLastError();
             }
         })
         return err;
@@ -495,9 +497,8 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
         if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int bpc;
             chunk_grid(nblocks, num_sms, occ, grid, bpc);
-            kern<<<grid, threads, smem, st>>>((const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
+            err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
                                               (const C*)twt, nblocks, bpc, m, sums);
-            err = cudaGetLastError();
         }
     })
     return err;
@@ -523,9 +524,8 @@ cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int
         if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
-            kern<<<grid, threads, smem, st>>>((const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks, (const C*)twt,
+            err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks, (const C*)twt,
                                               ngroups, gpc, mirror);
-            err = cudaGetLastError();
         }
     })
     return err;
@@ -551,9 +551,8 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
         if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
-            kern<<<grid, threads, smem, st>>>((const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks, (const C*)twt,
+            err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks, (const C*)twt,
                                               ngroups, gpc, mirror);
-            err = cudaGetLastError();
         }
     })
     return err;

@@ -2,12 +2,29 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stddef.h>
+#include <stdlib.h>
 #include <string>
 #include <vector>
 
 #include "../../include/hfft.h"
 
 namespace hfft {
+
+// Launch of a hot-path kernel with programmatic dependent launch (PDL): the kernel may start -- run its prologue:
+// index arithmetic, twiddle registers, shared-memory addresses -- while the previous kernel of the stream drains;
+// every such kernel executes pdl_wait() (fft.cuh: griddepcontrol.wait) before it touches data that kernel wrote.
+// Takes the launch gaps out of the five-kernel evaluation (B200, C3: 0.147 -> see DESIGN.md 8).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    static const int pdl_on = getenv("HFFT_NO_PDL") ? 0 : 1;      // HFFT_NO_PDL=1: plain stream order (A/B measurements)
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = pdl_on;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
 
 // per-layer saturation magnetisation, passed by value to the S1 kernel (hfft.h: "read during the
 // call and passed by value to the kernels")
