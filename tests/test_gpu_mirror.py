@@ -198,3 +198,34 @@ def test_mirror_automatic_mode_on_mid_size_grids(hb, prec, nx, ny):
     ref = O.hybrid_field(nx, ny, 3, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
     assert _relerr(H, ref) <= TOL[prec]
     plan.close()
+
+
+def test_storage_variants_agree_on_random_shapes(hb):
+    """Plain, mirror, mirror + reciprocity and class-indexed banks are storages of the same tensor: on 40 seeded random
+    shapes (ragged tiles, tiny and odd layer counts, batches) their fields agree to rounding order."""
+    import torch
+    rng = np.random.default_rng(20240607)
+    done = 0
+    while done < 40:
+        nx, ny = int(rng.choice([2, 4, 8, 16, 32, 64, 128])), int(rng.choice([2, 4, 8, 16, 32, 64]))
+        nz, B = int(rng.integers(1, 41)), int(rng.choice([1, 1, 2, 3]))
+        prec = str(rng.choice(["f32", "f64"]))
+        if nx * ny * nz * B > 4e5:
+            continue
+        done += 1
+        dz = np.exp(rng.uniform(np.log(0.3), np.log(3.0), size=nz))
+        Ms = 8e5 * (0.5 + rng.uniform(size=nz))
+        dt = torch.float32 if prec == "f32" else torch.float64
+        m = torch.randn(B, 3, nz, ny, nx, device="cuda", dtype=dt)
+        m /= m.norm(dim=1, keepdim=True)
+        fields = {}
+        for name, kw in [("plain", dict(dedup=0, mirror=0)), ("mirror", dict(dedup=0, mirror=2)),
+                         ("recip", dict(dedup=0, mirror=2, recip=1)), ("classes", dict(dedup=2, mirror=0))]:
+            plan = hb.Plan(nx, ny, nz, 2.0, 1.5, dz, prec, batch=B, **kw)
+            plan.build_tensor()
+            fields[name] = plan.demag(m, Ms).double().cpu().numpy()
+            plan.close()
+        ref = fields["plain"]
+        assert np.isfinite(ref).all()
+        for name, H in fields.items():
+            assert _relerr(H, ref) <= (1e-6 if prec == "f32" else 1e-13), (name, nx, ny, nz, B, prec)
