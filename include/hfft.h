@@ -22,6 +22,14 @@
  * is no cuFFT, no CPU fallback and no collective.  Every call returns a status;
  * nothing throws across this boundary.  A plan is not thread-safe.
  *
+ * Storage of the spectral tensor bank -- all give the same field, chosen automatically
+ * from the geometry, each switchable before hfft_build_tensor:
+ *   plain        one entry per (layer pair, wavevector)
+ *   ky mirror    hfft_plan_set_mirror: ky and 2ny-ky share an entry (default on large grids)
+ *   reciprocity  hfft_plan_set_recip: layer pairs p <= q only (memory, not speed; default off)
+ *   classes      hfft_plan_set_dedup: one entry per distinct (dz_i, dz_j, Z_ij); for equal
+ *                thicknesses the Toeplitz form or the z-convolution by FFT (Eq.25)
+ *
  * Array layout (all calls): [B][3][nz][ny][nx], x fastest, component order
  * (x,y,z), element type float (HFFT_F32) or double (HFFT_F64), 16-byte aligned.
  */
