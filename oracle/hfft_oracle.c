@@ -230,8 +230,10 @@ double hfft_oracle_nxx_fp64(const double X[3], const double D[3], const double D
 /* on the lattice (P dx, Q dy, zeta_a - zeta_b), P in [-nx,nx],          */
 /* Q in [-ny,ny], a in {i,i+1}, b in [0,nz].  phi() below memoises       */
 /* f/g on that lattice; |P|,|Q| are stored and the sign restored from   */
-/* the parity of Eq.10/16 in that argument (tested in test_oracle_newell */
-/* and against hfft_oracle_tensor_point on negative offsets).            */
+/* the parity of Eq.10/16 in that argument.  Pinned entry by entry,      */
+/* negative offsets included, against hfft_oracle_tensor_point by        */
+/* tests/test_oracle_newell.py::test_tensor_row_equals_tensor_point_on_  */
+/* every_entry (comment only; arithmetic unchanged).                     */
 /* ------------------------------------------------------------------ */
 typedef struct {
     int nx, ny, nz;

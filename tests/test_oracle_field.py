@@ -130,3 +130,54 @@ def test_paper_worked_example_saf_thickness():
             break
     assert abs(t1 - t_paper) < tol, t1
     assert round(t1, 2) == t_paper
+
+
+# ---------------------------------------------------------------- off-diagonal plumbing of T0 / T1
+@pytest.mark.parametrize("src,tgt", [((1, 2, 0), (10, 8, 2)), ((9, 1, 2), (0, 7, 0)), ((3, 8, 1), (11, 0, 2))])
+def test_single_cell_source_gives_every_field_component_in_another_layer(src, tgt):
+    """One cell of layer j magnetised along b = x, y, z in turn; all three components of H in a distant cell of
+    another layer i, from T0 (direct_field) and T1 (hybrid_field):
+
+      H_a(target) = - Ms_j N^{ab}_{ij}((a1-b1) dx, (a2-b2) dy) m_b           (Eq.18, one term)
+
+    (a) against hfft_oracle_tensor_point evaluated here at the offset (X, Y, zeta_i - zeta_j) with the symmetric
+        3 x 3 tensor written out from its six components (Eq.4) -- pins the component table COMP of
+        oracle.py / hfft_oracle.c and the sign and index conventions of the off-diagonal entries, which no
+        uniform-magnetisation or zz-only test sees;
+    (b) against the point-dipole field of Eq.1-2, H = (3 r (r.mu) - mu r^2) / (4 pi r^5),
+        mu = Ms V' m, r from the source centre to the target centre: relative deviation O((cell / r)^2)."""
+    nx, ny, nz = 12, 10, 3
+    dx, dy = 1.0, 1.2
+    dz = np.array([0.7, 1.6, 1.1])
+    Ms = np.array([8e5, 1.1e6, 9e5])
+    zeta = np.concatenate([[0.0], np.cumsum(dz)])
+    (b1, b2, j), (a1, a2, i) = src, tgt
+    assert i != j
+    X = np.array([(a1 - b1) * dx, (a2 - b2) * dy, zeta[i] - zeta[j]])
+    hi, lo = O.tensor_point(X, [dx, dy, dz[i]], [dx, dy, dz[j]])
+    n = hi + lo
+    xx, yy, zz, xy, xz, yz = n
+    N = np.array([[xx, xy, xz], [xy, yy, yz], [xz, yz, zz]])
+    assert min(abs(xy), abs(xz), abs(yz)) > 1e-6                 # generic offset: no component vanishes
+    # centre-to-centre vector and the dipole tensor (1 / 4 pi) (3 r r^T / r^5 - I / r^3)
+    r = X + 0.5 * np.array([0.0, 0.0, dz[i] - dz[j]])
+    rn = np.linalg.norm(r)
+    dip = (3.0 * np.outer(r, r) / rn**5 - np.eye(3) / rn**3) / (4.0 * np.pi)
+    Vp = dx * dy * dz[j]
+    for b in range(3):
+        m = np.zeros((3, nz, ny, nx))
+        m[b, j, b2, b1] = 1.0
+        want = -Ms[j] * N[:, b]
+        H0 = O.direct_field(nx, ny, nz, dx, dy, dz, m, Ms)
+        H1 = O.hybrid_field(nx, ny, nz, dx, dy, dz, m, Ms, dft="fft")
+        for H in (H0, H1):
+            got = H[:, i, a2, a1]
+            assert np.abs(got - want).max() <= 1e-13 * np.abs(Ms[j] * n).max(), (b, got, want)
+        # dipole limit: sign and position of every off-diagonal entry, independent of the Newell formulas
+        mu = np.zeros(3)
+        mu[b] = Ms[j] * Vp
+        Hd = dip @ mu
+        assert np.abs(H0[:, i, a2, a1] - Hd).max() <= 0.05 * np.abs(Hd).max(), (b, H0[:, i, a2, a1], Hd)
+        for a in range(3):
+            if abs(Hd[a]) > 0.2 * np.abs(Hd).max():
+                assert np.sign(H0[a, i, a2, a1]) == np.sign(Hd[a])

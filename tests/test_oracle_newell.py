@@ -342,3 +342,58 @@ def test_binary128_is_needed():
     assert errs[0] < 1e-9
     assert errs[2] > 1e-6          # fp64 has lost most digits at 250 cells
     assert errs[2] > 100 * errs[0]
+
+
+# ---------------------------------------------------------------- lattice-memo path of tensor_row
+def test_tensor_row_equals_tensor_point_on_every_entry():
+    """hfft_oracle_tensor_row (lattice memo: its own parity tables PAR_X / PAR_Y, its own ROLE permutations
+    and `shift` logic, a second transcription of PAPER.md:46 and :99 / Eq.5, 11, 19 :150) against
+    hfft_oracle_tensor_point (pinned above by quadrature, dipole limit, Aharoni, trace, additivity,
+    reciprocity): all six components, every target i and source j, every in-plane offset p, q including
+    the negative ones; unequal dz, nx != ny, dx != dy.  Mutations tried against this test:
+    a sign on PAR_X[4] or PAR_Y[5], a sign on the memoised g, and exchanging the argument permutations of xz and
+    yz in phi_eval all FAIL here.  Permuting ROLE[c] cannot fail anything: the nested sums of Eq.5 x 28 x 27 and
+    Eq.11 x 31 x 30 are a product of one four-point stencil per physical axis, so which axis plays which of the
+    paper's roles does not change the result (an equivalent mutant, like exchanging a and b in `shift`)."""
+    nx, ny, nz = 8, 4, 4
+    dx, dy = 1.7, 0.9
+    dz = np.array([1.0, 2.3, 0.6, 1.45])
+    zeta = np.concatenate([[0.0], np.cumsum(dz)])
+    worst = 0.0
+    scale = 0.0
+    for i in range(nz):
+        row = O.tensor_row(nx, ny, nz, dx, dy, dz, i)
+        assert row.shape == (nz, 6, 2 * ny - 1, 2 * nx - 1)
+        for j in range(nz):
+            D, Dp = [dx, dy, dz[i]], [dx, dy, dz[j]]
+            for q in range(-(ny - 1), ny):
+                for p in range(-(nx - 1), nx):
+                    # Z_ij = zeta_i - zeta_j (lower faces, reading A8), formed exactly as the sum of whole layers
+                    Z = float(sum(dz[j:i])) if i >= j else -float(sum(dz[i:j]))
+                    assert abs(Z - (zeta[i] - zeta[j])) < 1e-15
+                    hi, lo = O.tensor_point([p * dx, q * dy, Z], D, Dp)
+                    got = row[j, :, q + ny - 1, p + nx - 1]
+                    worst = max(worst, float(np.abs(got - (hi + lo)).max()))
+                    scale = max(scale, float(np.abs(hi).max()))
+    # both paths are binary128 rounded once to fp64; they differ by the rounding of p*dx, of zeta (a few ulp
+    # of the arguments) and of the final value
+    assert scale > 0.1 and worst <= 1e-15 * max(scale, 1.0), worst
+
+
+def test_tensor_row_off_diagonal_signs_under_offset_reversal():
+    """R4 on the row itself: xy odd in X and Y, xz odd in X / even in Y, yz even in X / odd in Y, diagonals
+    even -- read straight from the stored negative offsets (the PAR_X / PAR_Y tables), with values that are
+    not small (so a wrong sign cannot hide in rounding)."""
+    nx, ny, nz = 6, 5, 3
+    dz = np.array([0.8, 1.9, 1.1])
+    row = O.tensor_row(nx, ny, nz, 1.3, 1.1, dz, 1)
+    cx, cy = nx - 1, ny - 1
+    sx = [1, 1, 1, -1, -1, 1]
+    sy = [1, 1, 1, -1, 1, -1]
+    for j in (0, 2):
+        for c in range(6):
+            a = row[j, c]
+            assert np.abs(a).max() > 1e-4
+            assert np.abs(a[:, ::-1] - sx[c] * a).max() <= 1e-16, (j, c)
+            assert np.abs(a[::-1, :] - sy[c] * a).max() <= 1e-16, (j, c)
+            assert np.abs(a[cy + 1, cx + 2]) > 1e-5      # a generic offset is non-zero for every component
