@@ -568,6 +568,10 @@ template <typename T>
 cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st) {
     constexpr int KV = 16 / sizeof(T);
     if (a.zfft) return launch_coupling_zfft<T>(a, st);
+    if (a.symv) {
+        if constexpr (sizeof(T) == 4) return launch_coupling_symv(a, st);
+        else return cudaErrorInvalidValue;
+    }
     if (a.mirror && a.recip) return a.tile_k == 64 ? launch_coupling_k<T, 2, true, true>(a, st) : cudaErrorInvalidValue;
     if (a.cls) {
         if (a.class_kernel) return a.tile_k == 32 ? launch_coupling_class<T>(a, st) : cudaErrorInvalidValue;

@@ -6,6 +6,7 @@
 #include <new>
 
 #include "hfft_internal.h"
+#include "symv_layout.h"
 
 using namespace hfft;
 
@@ -41,8 +42,9 @@ struct hfft_plan {
     // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
     int dedup_mode = 1;                              // 0 off, 1 auto, 2 on, 3 z-FFT (Eq.25)
     bool dedup = false, toeplitz = false, class_kernel = false;
-    int recip_mode = 0;                              // hfft_plan_set_recip
-    bool recip = false;                              // bank holds dz_p R_pq for p <= q only (with the mirror storage)
+    int recip_mode = 2;                              // hfft_plan_set_recip: 0 off, 1 on, 2 automatic
+    bool recip = false;                              // bank holds dz_p R_pq for one orientation of every pair (with the mirror storage)
+    bool symv = false;                               // ... in the symv layout, read once by coupling_symv_kernel
     std::vector<int> recip_cls, recip_rep;           // pair -> slot of the unordered pair; slot -> p*nz+q (p <= q)
     void* d_invdz = nullptr;                         // 1 / dz_i, plan precision (recip)
     int mirror_mode = 1;                             // hfft_plan_set_mirror: 0 off, 1 automatic
@@ -153,6 +155,7 @@ static BuildGeom make_geom(const hfft_plan* p) {
     BuildGeom g{p->nx, p->ny, p->nz, p->log2nx, p->log2ny, p->dx, p->dy, p->dz.data(),
                 p->tile_k, p->n_k, p->n_k_padded, p->prec, p->num_sms};
     g.mirror = p->mirror;
+    g.symv = p->symv; g.symv_bank_bytes = p->symv ? p->bank_bytes : 0;
     if (p->dedup) { g.pair_class = p->pair_class.data(); g.class_rep = p->class_rep.data(); g.n_classes = p->n_classes; }
     if (p->recip) {
         g.pair_class = p->recip_cls.data(); g.class_rep = p->recip_rep.data(); g.n_classes = (int)p->recip_rep.size();
@@ -200,23 +203,39 @@ static void plan_sizes(hfft_plan* p) {
     p->mirror = p->mirror_mode >= 1 && !p->dedup && (big || p->mirror_mode == 2) && p->ny >= 2 &&
                 !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
     if (p->mirror) p->tile_k = 64;
-    p->recip = p->mirror && p->recip_mode == 1 && p->nz >= 2 && p->nz * (p->nz + 1) / 2 <= 65535;
-    if (p->recip && p->recip_rep.empty()) {
+    // reciprocity storage on top of the mirror storage.  fp32, nz <= 64: the symv layout, every block read
+    // once and used for both of its layer pairs (coupling_symv.cu) -- automatic where it streams at least 30 % fewer
+    // bytes than the mirror bank (the layout pads nz to whole strips of 4 and the strips to a power of two);
+    // otherwise (mode 1 only) the p <= q storage read through the class table of the streaming kernel.
+    p->symv = false;
+    if (p->mirror && p->recip_mode >= 1 && coupling_symv_applies(p->nz, e)) {
+        const SymvGeom G = symv_geom(p->nz);
+        const bool wins = symv_pairs_per_entry(G) * 10 <= (long long)p->nz * p->nz * 7;
+        p->symv = p->recip_mode == 1 || wins;
+    }
+    p->recip = p->symv || (p->mirror && p->recip_mode == 1 && p->nz >= 2 && p->nz * (p->nz + 1) / 2 <= 65535);
+    p->recip_cls.clear(); p->recip_rep.clear();
+    if (p->recip) {
+        // slot of the unordered pair and its stored orientation (p, q): S_pq = dz_p R_pq; (q, p) is its transpose
         const int nz = p->nz;
+        const SymvGeom G = symv_geom(nz);
         p->recip_cls.assign((size_t)nz * nz, 0);
         for (int a = 0; a < nz; ++a)
             for (int b = a; b < nz; ++b) {
                 const int slot = (int)p->recip_rep.size();
-                p->recip_rep.push_back(a * nz + b);
+                const bool swap = p->symv && symv_pos(G, a, b).transposed;
+                p->recip_rep.push_back(swap ? b * nz + a : a * nz + b);
                 p->recip_cls[(size_t)a * nz + b] = p->recip_cls[(size_t)b * nz + a] = slot;
             }
     }
+    if (p->symv) p->tile_k = 2 * coupling_symv_tile_entries(p->nz);
     p->n_slots = p->mirror ? (long long)(p->nx + 1) * (2 * p->ny + 2) : p->n_k;
     p->n_tiles = (p->n_slots + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
     const size_t slots = p->zfft ? ((size_t)1 << p->log2lz)
                          : (p->recip ? (size_t)p->nz * (p->nz + 1) / 2 : (p->dedup ? p->n_classes : p->nz * p->nz));
     p->bank_bytes = (size_t)6 * slots * (size_t)(p->mirror ? p->n_k_padded / 2 : p->n_k_padded) * e;
+    if (p->symv) p->bank_bytes = coupling_symv_bank_bytes(p->nz, p->n_tiles);
     const size_t planes = (size_t)3 * p->nz * p->batch;
     auto al = [](size_t v) { return (v + 255) & ~(size_t)255; };
     size_t o = 0;
@@ -312,7 +331,7 @@ hfft_status hfft_plan_set_mirror(hfft_plan* plan, int on) {
 
 hfft_status hfft_plan_set_recip(hfft_plan* plan, int on) {
     if (!plan) return HFFT_EINVAL;
-    if (on != 0 && on != 1) return fail(plan, HFFT_EINVAL, "hfft_plan_set_recip: 0 or 1");
+    if (on < 0 || on > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_recip: 0, 1 or 2");
     if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_recip: after build / set_buffers");
     plan->recip_mode = on;
     plan_sizes(plan);
@@ -343,7 +362,7 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->launches_per_demag = HFFT_NUM_STAGES;
     info->built = plan->built ? 1 : 0;
     info->n_classes = plan->n_classes;
-    info->mirror = plan->mirror ? (plan->recip ? 2 : 1) : 0;
+    info->mirror = plan->mirror ? (plan->symv ? 3 : (plan->recip ? 2 : 1)) : 0;
     info->dedup = plan->zfft ? 4 : (plan->dedup ? (plan->class_kernel ? (plan->toeplitz ? 3 : 2) : 1) : 0);
     return HFFT_OK;
 }
@@ -460,7 +479,7 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
     CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
                     p->recip ? (int)p->recip_rep.size() : (p->dedup ? p->n_classes : p->nz * p->nz),
                     (p->dedup || p->recip) ? p->d_cls : nullptr, p->class_kernel, p->toeplitz, p->num_sms};
-    ca.recip = p->recip; ca.inv_dz = p->d_invdz;
+    ca.recip = p->recip; ca.inv_dz = p->d_invdz; ca.symv = p->symv;
     ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz; ca.mirror = p->mirror;
     STAGE(2, (launch_coupling<T>(ca, st)))
     STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st,
@@ -645,6 +664,32 @@ hfft_status hfft_read_bank(const hfft_plan* plan, int i, int j, int c, double* o
     // reciprocity storage: the slot of the unordered pair holds dz_p R_pq (p <= q); (q, p) is its transpose
     const double unscale = -4.0 * p->nx * p->ny * ((p->dedup && p->toeplitz && i < j && c >= 4) ? -1.0 : 1.0) *
                            (p->recip ? ((i > j && c >= 4) ? -1.0 : 1.0) / p->dz[i] : 1.0);
+    if (p->symv) {
+        // symv layout: one float per bank entry, strided by the unit's stream (symv_layout.h); the stored orientation
+        // holds dz_p R_pq, the other one is its transpose (xz, yz negated)
+        const SymvGeom G = symv_geom(p->nz);
+        const SymvPos pos = symv_pos(G, i, j);
+        const double us = -4.0 * p->nx * p->ny * ((pos.transposed && c >= 4) ? -1.0 : 1.0) / p->dz[i];
+        const long long n_units = (n_e + G.EPW - 1) / G.EPW;
+        const size_t unit_bytes = (size_t)G.NC * kSymvCoupleBytes;
+        std::vector<float> col((size_t)n_units);
+        for (int ent = 0; ent < G.EPW; ++ent) {
+            const size_t off = (size_t)symv_float_offset(G, pos, ent, c) * sizeof(float);
+            e = cudaMemcpy2D(col.data(), sizeof(float), static_cast<unsigned char*>(p->bank) + off, unit_bytes, sizeof(float),
+                             (size_t)n_units, cudaMemcpyDeviceToHost);
+            if (e != cudaSuccess) return fail_cuda(p, "cudaMemcpy2D(bank)", e);
+            for (long long u = 0; u < n_units; ++u) {
+                const long long en = u * G.EPW + ent;
+                if (en >= n_e) break;
+                const double v = (double)col[(size_t)u] * us;
+                const long long kx = en / (p->ny + 1);
+                const int ty = (int)(en - kx * (p->ny + 1));
+                out_host[kx * 2 * p->ny + ty] = v;
+                if (ty > 0 && ty < p->ny) out_host[kx * 2 * p->ny + (2 * p->ny - ty)] = (c == 3 || c == 5) ? -v : v;
+            }
+        }
+        return HFFT_OK;
+    }
     std::vector<unsigned char> buf((size_t)tk * p->elem);
     for (long long t = 0; t < p->n_tiles; ++t) {
         const size_t ncls = p->recip ? p->recip_rep.size() : (p->dedup ? p->n_classes : (size_t)p->nz * p->nz);

@@ -3,7 +3,10 @@
 #include <cuda_runtime.h>
 #include <stddef.h>
 #include <stdlib.h>
+#include <map>
+#include <mutex>
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/hfft.h"
@@ -24,6 +27,46 @@ inline cudaError_t launch_pdl(void (*kern)(KArgs...), dim3 grid, dim3 block, siz
     at[0].val.programmaticStreamSerializationAllowed = pdl_on;
     cfg.attrs = at; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, kern, static_cast<KArgs>(args)...);
+}
+
+// Launch attributes are properties of a (kernel, device) pair: the opt-in to more than 48 KB of dynamic shared memory
+// (cudaFuncSetAttribute) and the occupancy the runtime reports.  Every launcher keeps them in one of these caches,
+// keyed by device ordinal and a launcher-defined key (threads, shared-memory bytes), guarded by a mutex, so that
+// plans on several devices or host threads of one process do not share stale values.
+template <typename V> class PerDevice {
+  public:
+    bool get(int dev, long long key, V& out) {
+        std::lock_guard<std::mutex> lock(mu_);
+        auto it = map_.find(std::make_pair(dev, key));
+        if (it == map_.end()) return false;
+        out = it->second;
+        return true;
+    }
+    void set(int dev, long long key, const V& v) {
+        std::lock_guard<std::mutex> lock(mu_);
+        map_[std::make_pair(dev, key)] = v;
+    }
+  private:
+    std::mutex mu_;
+    std::map<std::pair<int, long long>, V> map_;
+};
+
+// CTAs per SM of `kernel` launched with (threads, smem) on the current device, opting in to smem > 48 KB first
+template <typename K>
+inline cudaError_t ctas_per_sm_cached(K kernel, int threads, size_t smem, PerDevice<int>& cache, int& occ) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    const long long key = ((long long)threads << 32) | (long long)smem;
+    if (cache.get(dev, key, occ)) return cudaSuccess;
+    if (smem > 48 * 1024 &&
+        (e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+        return e;
+    int nb = 0;
+    if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, smem)) != cudaSuccess) return e;
+    occ = nb < 1 ? 1 : nb;
+    cache.set(dev, key, occ);
+    return cudaSuccess;
 }
 
 // per-layer saturation magnetisation, passed by value to the S1 kernel (hfft.h: "read during the
@@ -68,12 +111,19 @@ struct CouplingArgs {
     bool recip = false;            // reciprocity storage: cls = slot of the unordered pair, bank = dz_p R_pq (p <= q)
     const void* inv_dz = nullptr;  // device, [nz] plan precision (recip)
     bool mirror = false;           // spectrum in the mirror layout, one bank value per pair of slots (coupling_kernel MIR)
+    bool symv = false;             // reciprocity bank in the symv layout (coupling_symv.cu, symv_layout.h); fp32
     bool zfft = false;
     int log2lz = 0;
     const void* twz = nullptr;     // device, exp(-2 pi i n / Lz), plan precision
 };
 template <typename T>
 cudaError_t launch_coupling(const CouplingArgs& a, cudaStream_t st);
+// ---- coupling_symv.cu ----
+constexpr int kSymvWarps = 8;      // warps per CTA of coupling_symv_kernel; a CTA tile is kSymvWarps * EPW bank entries
+bool coupling_symv_applies(int nz, size_t elem);
+int coupling_symv_tile_entries(int nz);
+size_t coupling_symv_bank_bytes(int nz, long long n_tiles);
+cudaError_t launch_coupling_symv(const CouplingArgs& a, cudaStream_t st);
 // ---- coupling_zfft.cu ----
 template <typename T>
 cudaError_t launch_coupling_zfft(const CouplingArgs& a, cudaStream_t st);
@@ -101,6 +151,8 @@ struct BuildGeom {
     // i*nz+j [n_classes]; pair_class == nullptr: one slot per pair (class = i*nz+j)
     bool mirror = false;   // bank entry p = kx * (ny + 1) + t, t = 0..ny, serves ky = t and ky = 2ny - t; tile_k / 2 per tile
     bool recip = false;    // bank value of the representative pair (p, q), p <= q, is multiplied by dz_p
+    bool symv = false;     // recip in the symv layout (symv_layout.h): tile_k / 2 entries per CTA tile of kSymvWarps units
+    size_t symv_bank_bytes = 0;
     const int* pair_class = nullptr;
     const int* class_rep = nullptr;
     int n_classes = 0;

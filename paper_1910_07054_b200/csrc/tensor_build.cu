@@ -27,6 +27,7 @@
 
 #include "hfft_internal.h"
 #include "newell_dd.cuh"
+#include "symv_layout.h"
 
 namespace hfft {
 
@@ -151,6 +152,26 @@ pack_kernel(T* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, 
     } else {
         bank[blk + (long long)c * tile_e + kk] = (T)v;
     }
+}
+
+// Reciprocity bank in the symv layout (symv_layout.h): the pairs (i, j0 + jl) of a run are stored orientations, their
+// value S_ij = dz_i R_ij (the factor is in `scale`) goes to [unit = e / EPW][couple][...] for bank entry e = kx (ny + 1) + t.
+__global__ void __launch_bounds__(256)
+pack_symv_kernel(float* __restrict__ bank, const double2* __restrict__ Y, int nz, int i, int j0, long long n_k, long long n_e,
+                 int ny, double scale) {
+    const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int jc = blockIdx.y;          // jl * 6 + c
+    if (e >= n_e) return;               // padding entries and padding rows stay zero (the bank is cleared first)
+    const int jl = jc / 6, c = jc - jl * 6;
+    const SymvGeom G = symv_geom(nz);
+    const SymvPos pos = symv_pos(G, i, j0 + jl);
+    const long long kx = e / (ny + 1);
+    const long long k = kx * 2 * ny + (e - kx * (ny + 1));
+    const double2 t = Y[(size_t)jc * n_k + k];
+    const double v = (c < 4 ? t.x : t.y) * scale;
+    const long long unit = e / G.EPW;
+    const int ent = (int)(e - unit * G.EPW);
+    bank[unit * G.NC * kSymvCoupleFloats + symv_float_offset(G, pos, ent, c)] = (float)v;
 }
 
 struct ScratchLayout {
@@ -291,6 +312,8 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
     const int ncls = g.pair_class ? g.n_classes : nz * nz;
     HFFT_CK(cudaStreamSynchronize(st));   // `zeta`, `cls16` are pageable host memory
     HFFT_CK(cudaMemsetAsync(d_R, 0, (size_t)L.jc * 6 * 4 * nx * ny * 8, st));   // slots p = nx, q = ny stay 0
+    // symv layout: padding rows (nz not a multiple of 4), idle strip-lanes and padding entries hold zeros
+    if (g.symv && changed < 0) HFFT_CK(cudaMemsetAsync(bank, 0, g.symv_bank_bytes, st));
 
     const double scale = -1.0 / (4.0 * (double)nx * (double)ny);
     const dd inv4pi = dd_make(DD_INV_4PI_HI, DD_INV_4PI_LO);
@@ -337,7 +360,10 @@ cudaError_t build_bank(const BuildGeom& g, void* bank, void* scratch, const void
                 const long long n_e = g.mirror ? (long long)(nx + 1) * (ny + 1) : g.n_k;
                 const long long n_e_padded = g.mirror ? g.n_k_padded / 2 : g.n_k_padded;
                 dim3 gridp((unsigned)((n_e_padded + 255) / 256), jn * 6);
-                if (g.prec == HFFT_F32)
+                if (g.symv)
+                    pack_symv_kernel<<<dim3((unsigned)((n_e + 255) / 256), jn * 6), 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, g.n_k,
+                                                                                              n_e, ny, pscale);
+                else if (g.prec == HFFT_F32)
                     pack_kernel<float><<<gridp, 256, 0, st>>>((float*)bank, d_Y, nz, i, j0, ncls, d_cls, tile_e, g.n_k, n_e,
                                                               n_e_padded, g.mirror ? ny : 0, pscale);
                 else

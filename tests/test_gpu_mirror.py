@@ -135,9 +135,12 @@ def test_reciprocity_storage_vs_oracle(hb, nx, ny, nz, B, prec):
     info = hb.plan_info(plan.handle)
     batched_kernel = B > 1 and 6 * nz * (4 if prec == "f32" else 8) <= 384
     too_many_layers = 3 * nz * 64 * (8 if prec == "f32" else 16) > 200 * 1024      # the M^ tile must fit shared memory
-    assert info.mirror == (0 if batched_kernel or too_many_layers else 2)
+    symv = prec == "f32" and nz <= 64                       # fp32, at most 16 strips of 4 layers: the symv layout
+    assert info.mirror == (0 if batched_kernel or too_many_layers else (3 if symv else 2))
     if info.mirror == 2:
         assert info.bank_bytes == 6 * (nz * (nz + 1) // 2) * (info.n_k_padded // 2) * (4 if prec == "f32" else 8)
+    if info.mirror == 3:
+        assert info.bank_bytes == (info.n_k_padded // info.tile_k) * 8 * _symv_couples(nz) * 768
     dt = torch.float32 if prec == "f32" else torch.float64
     H = plan.demag(torch.from_numpy(m).to(dt).cuda(), w.Ms).double().cpu().numpy()
     ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
@@ -146,6 +149,88 @@ def test_reciprocity_storage_vs_oracle(hb, nx, ny, nz, B, prec):
         ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, w.dz, m[0], w.Ms)
         assert _relerr(H[0], ref0) <= TOL[prec]
     plan.close()
+
+
+def _symv_couples(nz):
+    """Couples (two stored layer pairs for each of 16 strip-lanes, 768 bytes) in a warp-unit's stream: symv_layout.h."""
+    W = (nz + 3) // 4
+    return 8 * ((W - 1) // 2) + 4 * (1 if W >= 2 and W % 2 == 0 else 0) + 5
+
+
+@pytest.mark.parametrize("nx,ny,nz,B", [(8, 8, 2, 1), (16, 4, 4, 1), (8, 16, 5, 1), (16, 16, 8, 1), (8, 8, 9, 1),
+                                        (4, 16, 12, 1), (16, 8, 16, 1), (8, 4, 17, 1), (8, 8, 24, 1), (4, 8, 27, 2),
+                                        (8, 8, 32, 1), (4, 4, 33, 1), (8, 4, 48, 1), (4, 8, 61, 1), (8, 8, 64, 1),
+                                        (64, 32, 20, 1), (32, 16, 40, 3)])
+def test_symv_reciprocity_kernel_vs_oracle(hb, nx, ny, nz, B):
+    """coupling_symv_kernel (fp32 reciprocity bank, every block used for both of its layer pairs): every strip count
+    W = 1..16, odd and even (with and without the half block), layer counts that are not multiples of 4 (padding
+    rows), idle strip-lanes (W not a power of two), several entries per warp, ragged last tile, batches."""
+    import torch
+    w = W.small(nx, ny, nz, precision="f32", B=B, seed=2900 + nx + 3 * ny + 7 * nz)
+    m = w.m_rounded()
+    plan = hb.Plan(nx, ny, nz, w.dx, w.dy, w.dz, "f32", batch=B, dedup=0, mirror=2, recip=1)
+    plan.build_tensor()
+    info = hb.plan_info(plan.handle)
+    assert info.mirror == 3
+    md = torch.from_numpy(m).float().cuda()
+    for _ in range(2):                                   # second call: padding and dummy slots still hold zeros
+        H = plan.demag(md, w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(nx, ny, nz, w.dx, w.dy, w.dz, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f32"]
+    if nx * ny * nz <= 2048:
+        ref0 = O.direct_field(nx, ny, nz, w.dx, w.dy, w.dz, m[0], w.Ms)          # the definition, Eq.18
+        assert _relerr(H[0], ref0) <= TOL["f32"]
+    plan.close()
+
+
+def test_symv_bank_reads_back_like_the_plain_bank(hb):
+    """hfft_read_bank through the symv layout: every ordered pair (stored orientation or its transpose) of a stack
+    with a half block (W = 2) and one with full blocks and idle strip-lanes (W = 5)."""
+    for nz in (7, 18):
+        w = W.small(16, 8, nz, precision="f32", seed=14 + nz)
+        a = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, w.dz, "f32", dedup=0, mirror=0)
+        b = hb.Plan(w.nx, w.ny, nz, w.dx, w.dy, w.dz, "f32", dedup=0, mirror=2, recip=1)
+        a.build_tensor()
+        b.build_tensor()
+        assert hb.plan_info(b.handle).mirror == 3
+        worst = 0.0
+        for i in range(nz):
+            for j in range(nz):
+                for c in range(6):
+                    x, y = hb.read_bank(a.handle, i, j, c), hb.read_bank(b.handle, i, j, c)
+                    worst = max(worst, np.abs(x - y).max() / max(np.abs(x).max(), 1e-30))
+        assert worst <= 2e-6, (nz, worst)
+        a.close()
+        b.close()
+
+
+def test_symv_with_update_dz_and_reductions(hb):
+    import torch
+    w = W.small(32, 16, 9, precision="f32", seed=36)
+    dz2 = w.dz.copy()
+    dz2[4] = 0.9
+    plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, "f32", dedup=0, mirror=2, recip=1)
+    plan.build_tensor()
+    assert hb.plan_info(plan.handle).mirror == 3
+    plan.update_dz(4, 0.9)
+    sums = plan.set_reduction(True)
+    m = w.m_rounded()
+    H = plan.demag(torch.from_numpy(m).float().cuda(), w.Ms).double().cpu().numpy()
+    ref = O.hybrid_field(w.nx, w.ny, w.nz, w.dx, w.dy, dz2, m, w.Ms, dft="fft")
+    assert _relerr(H, ref) <= TOL["f32"]
+    assert np.abs(sums.cpu().numpy()[..., 0] - ref.sum(axis=(-1, -2))).max() <= 2e-6 * np.abs(ref).max() * w.nx * w.ny
+    plan.close()
+
+
+def test_symv_automatic_mode(hb):
+    """Default plans: the symv bank is chosen where the mirror storage is and it streams at least 30 % fewer bytes."""
+    for nz, want in ((16, 3), (64, 3), (3, 1), (20, 1)):
+        q = hb.Plan(256, 256, nz, 2.0, 2.0, np.exp(np.linspace(-0.5, 0.7, nz)), "f32", torch_buffers=False)
+        assert hb.plan_info(q.handle).mirror == want, (nz, hb.plan_info(q.handle).mirror)
+        q.close()
+    q = hb.Plan(256, 256, 16, 2.0, 2.0, np.exp(np.linspace(-0.5, 0.7, 16)), "f64", torch_buffers=False)
+    assert hb.plan_info(q.handle).mirror == 1            # fp64: mirror storage only
+    q.close()
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
@@ -157,7 +242,7 @@ def test_reciprocity_bank_reads_back_like_the_plain_bank(hb, prec):
     b = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, prec, dedup=0, mirror=2, recip=1)
     a.build_tensor()
     b.build_tensor()
-    assert hb.plan_info(b.handle).mirror == 2
+    assert hb.plan_info(b.handle).mirror == (3 if prec == "f32" else 2)
     worst = 0.0
     for i in range(4):
         for j in range(4):
