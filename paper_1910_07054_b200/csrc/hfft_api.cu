@@ -204,13 +204,13 @@ static void plan_sizes(hfft_plan* p) {
                 !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
     if (p->mirror) p->tile_k = 64;
     // reciprocity storage on top of the mirror storage.  fp32, nz <= 64: the symv layout, every block read
-    // once and used for both of its layer pairs (coupling_symv.cu) -- automatic where it streams at least 30 % fewer
-    // bytes than the mirror bank (the layout pads nz to whole strips of 4 and the strips to a power of two);
+    // once and used for both of its layer pairs (coupling_symv.cu) -- automatic from 8 layers on where it streams at
+    // least 30 % fewer bytes than the mirror bank (the layout pads nz to whole strips of 4, the strips to a power of two);
     // otherwise (mode 1 only) the p <= q storage read through the class table of the streaming kernel.
     p->symv = false;
     if (p->mirror && p->recip_mode >= 1 && coupling_symv_applies(p->nz, e)) {
         const SymvGeom G = symv_geom(p->nz);
-        const bool wins = symv_pairs_per_entry(G) * 10 <= (long long)p->nz * p->nz * 7;
+        const bool wins = p->nz >= 8 && symv_pairs_per_entry(G) * 10 <= (long long)p->nz * p->nz * 7;
         p->symv = p->recip_mode == 1 || wins;
     }
     p->recip = p->symv || (p->mirror && p->recip_mode == 1 && p->nz >= 2 && p->nz * (p->nz + 1) / 2 <= 65535);

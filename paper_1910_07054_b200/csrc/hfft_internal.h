@@ -51,7 +51,10 @@ template <typename V> class PerDevice {
     std::map<std::pair<int, long long>, V> map_;
 };
 
-// CTAs per SM of `kernel` launched with (threads, smem) on the current device, opting in to smem > 48 KB first
+// CTAs per SM of `kernel` launched with (threads, smem) on the current device, opting in to smem > 48 KB first.
+// The opt-in is one attribute per (kernel, device) that every call overwrites: it is only ever raised (key -1 of the
+// cache holds the value in force), so that a launch whose occupancy is cached never finds it lowered by a later,
+// smaller configuration.
 template <typename K>
 inline cudaError_t ctas_per_sm_cached(K kernel, int threads, size_t smem, PerDevice<int>& cache, int& occ) {
     int dev = 0;
@@ -59,9 +62,13 @@ inline cudaError_t ctas_per_sm_cached(K kernel, int threads, size_t smem, PerDev
     if (e != cudaSuccess) return e;
     const long long key = ((long long)threads << 32) | (long long)smem;
     if (cache.get(dev, key, occ)) return cudaSuccess;
-    if (smem > 48 * 1024 &&
-        (e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
-        return e;
+    int opted = 48 * 1024;
+    cache.get(dev, -1, opted);
+    if ((int)smem > opted) {
+        if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
+            return e;
+        cache.set(dev, -1, (int)smem);
+    }
     int nb = 0;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, smem)) != cudaSuccess) return e;
     occ = nb < 1 ? 1 : nb;

@@ -224,7 +224,7 @@ def test_symv_with_update_dz_and_reductions(hb):
 
 def test_symv_automatic_mode(hb):
     """Default plans: the symv bank is chosen where the mirror storage is and it streams at least 30 % fewer bytes."""
-    for nz, want in ((16, 3), (64, 3), (3, 1), (20, 1)):
+    for nz, want in ((16, 3), (64, 3), (8, 3), (3, 1), (4, 1), (20, 1)):
         q = hb.Plan(256, 256, nz, 2.0, 2.0, np.exp(np.linspace(-0.5, 0.7, nz)), "f32", torch_buffers=False)
         assert hb.plan_info(q.handle).mirror == want, (nz, hb.plan_info(q.handle).mirror)
         q.close()
@@ -305,7 +305,7 @@ def test_storage_variants_agree_on_random_shapes(hb):
         m = torch.randn(B, 3, nz, ny, nx, device="cuda", dtype=dt)
         m /= m.norm(dim=1, keepdim=True)
         fields = {}
-        for name, kw in [("plain", dict(dedup=0, mirror=0)), ("mirror", dict(dedup=0, mirror=2)),
+        for name, kw in [("plain", dict(dedup=0, mirror=0)), ("mirror", dict(dedup=0, mirror=2, recip=0)),
                          ("recip", dict(dedup=0, mirror=2, recip=1)), ("classes", dict(dedup=2, mirror=0))]:
             plan = hb.Plan(nx, ny, nz, 2.0, 1.5, dz, prec, batch=B, **kw)
             plan.build_tensor()
