@@ -20,13 +20,17 @@
  *
  * Everything runs on ONE CUDA device (sm_100a), in hand-written kernels; there
  * is no cuFFT, no CPU fallback and no collective.  Every call returns a status;
- * nothing throws across this boundary.  A plan is not thread-safe.
+ * nothing throws across this boundary.  A plan is not thread-safe (one host thread
+ * at a time per plan); different plans may be used from different host threads and
+ * on different devices of one process (the per-kernel launch attributes the library
+ * caches are keyed by device and guarded by a mutex).
  *
  * Storage of the spectral tensor bank -- all give the same field, chosen automatically
  * from the geometry, each switchable before hfft_build_tensor:
  *   plain        one entry per (layer pair, wavevector)
  *   ky mirror    hfft_plan_set_mirror: ky and 2ny-ky share an entry (default on large grids)
- *   reciprocity  hfft_plan_set_recip: layer pairs p <= q only (memory, not speed; default off)
+ *   reciprocity  hfft_plan_set_recip: unordered layer pairs only, every 3 x 3 block read once and
+ *                used for both of its pairs (default from 8 layers on where the mirror storage is, fp32)
  *   classes      hfft_plan_set_dedup: one entry per distinct (dz_i, dz_j, Z_ij); for equal
  *                thicknesses the Toeplitz form or the z-convolution by FFT (Eq.25)
  *
@@ -52,7 +56,8 @@ typedef enum {
     HFFT_ENOMEM = 2,       /* device or host allocation failed */
     HFFT_ECUDA = 3,        /* a CUDA runtime call or kernel launch failed; see hfft_last_error */
     HFFT_ESTATE = 4,       /* call out of order (e.g. hfft_demag before hfft_build_tensor) */
-    HFFT_EUNSUPPORTED = 5  /* nx or ny not a power of two, nz above HFFT_MAX_NZ, no sm_100 device */
+    HFFT_EUNSUPPORTED = 5  /* nx or ny not a power of two or above 1024, nz above HFFT_MAX_NZ or too large for the
+                              coupling kernel's shared memory, no sm_100 device */
 } hfft_status;
 
 #define HFFT_MAX_NZ 256
@@ -71,16 +76,20 @@ typedef struct {
                                  multiple of tile_k */
     size_t bank_bytes;        /* spectral tensor bank: 6 * (nz^2 or n_classes) * n_k_padded * sizeof(element);
                                  half of that with mirror storage */
-    size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^) + host-path staging (two slots of m and h) */
+    size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^).  The host paths allocate their staging copies of
+                                 m and h themselves, on first use */
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
     int launches_per_demag;   /* kernels hfft_demag enqueues per call */
     int built;                /* 1 once hfft_build_tensor has completed */
     int n_classes;            /* bank slots a deduplicated bank needs: distinct tensors among the nz^2 layer pairs;
                                  nz for equal thicknesses (N_ij and N_ji then differ by the sign of xz, yz only) */
     int mirror;               /* 1: ky-mirror storage (hfft_plan_set_mirror): half the bank, spectrum rows of 2ny+2 slots;
-                                 2: with reciprocity storage on top (hfft_plan_set_recip): a quarter of the bank */
+                                 2: with reciprocity storage on top (hfft_plan_set_recip): a quarter of the bank, read
+                                    through a pair table; 3: reciprocity storage in the block layout of the
+                                    symmetric-matvec kernel (every block read once) */
     int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
-                                 shared memory; 3: as 2 with Toeplitz classes (equal thicknesses) */
+                                 shared memory; 3: as 2 with Toeplitz classes (equal thicknesses); 4: equal
+                                 thicknesses, z-convolution by FFT (Eq.25) */
 } hfft_info;
 
 /*
@@ -90,8 +99,11 @@ typedef struct {
  * any one unit (the tensor depends on ratios only).  Selects device = the
  * current CUDA device.  No device memory is allocated here.
  * Errors: EINVAL (null out/dz, nx,ny < 2, nz < 1, non-positive or non-finite
- * dx, dy, dz[k]); EUNSUPPORTED (nx or ny not a power of two, nz > HFFT_MAX_NZ,
- * device is not compute capability 10.x); ENOMEM.
+ * dx, dy, dz[k]); EUNSUPPORTED (nx or ny not a power of two; nx or ny > 1024, the
+ * longest row transform the FFT kernels hold in registers and shared memory;
+ * nz > HFFT_MAX_NZ; nz so large that the M^ tile of the coupling kernel (3 nz x 32
+ * wavevectors) exceeds 200 KB of shared memory, i.e. nz > 256 in fp32 and nz > 133
+ * in fp64; device is not compute capability 10.x); ECUDA (no CUDA device); ENOMEM.
  */
 hfft_status hfft_plan_create(hfft_plan **out, int nx, int ny, int nz,
                              double dx, double dy, const double *dz, hfft_precision precision);
@@ -111,10 +123,16 @@ hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
  * (info.bank_bytes shrinks by nz^2 / n_classes) and, where a k-tile of it fits in
  * shared memory, the coupling stage stops being HBM-bound (coupling.cu).
  *   mode 0: off (one slot per pair; required for hfft_update_dz)
- *   mode 1: automatic (default): on when n_classes <= nz^2 / 2
- *   mode 2: on
- * Results are those of the plain bank up to summation order.  Must be called
- * before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
+ *   mode 1: automatic (default): on when n_classes <= nz^2 / 2; equal thicknesses from 16
+ *           layers on use mode 3
+ *   mode 2: on (class kernel; Toeplitz form for equal thicknesses)
+ *   mode 3: equal thicknesses only: the z-convolution by FFT of PAPER.md:182 Eq.25 as stage S3
+ *           (zero-padded transforms of length 2^ceil(log2 2nz) along z at every in-plane
+ *           wavevector); needs 2 <= nz <= 128 (fp32) / 32 (fp64)
+ * info.dedup reports the kernel chosen.  Results are those of the plain bank up to summation
+ * order.  Must be called before hfft_build_tensor / hfft_plan_set_buffers.
+ * Errors: EINVAL (mode outside 0..3), ESTATE, EUNSUPPORTED (mode 3 on unequal thicknesses or
+ * outside its nz range).
  */
 hfft_status hfft_plan_set_dedup(hfft_plan *plan, int mode);
 
@@ -136,12 +154,20 @@ hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
 /*
  * Reciprocity storage of the bank, on top of the ky-mirror storage.
  * dz_i N_ij(X,Y) = dz_j N_ji(-X,-Y): in the real form of the coupling, S_ij := dz_i R_ij
- * satisfies S_ji = S_ij^T, so the bank keeps S_pq for p <= q only -- nz(nz+1)/2 instead
- * of nz^2 layer pairs, half the bytes again -- the pair (q, p) uses the transpose (xz, yz
- * negated) and H_i is multiplied by 1/dz_i at the end.  Every entry is then needed by two
- * target layers; the kernel orders its reads so that the second one is served by L2.
- * on = 1 takes effect wherever the mirror storage is active (info.mirror == 2 then);
- * default 0.  hfft_update_dz rebuilds the whole bank in this mode.  Must be called before
+ * satisfies S_ji = S_ij^T, so the bank keeps one 3 x 3 block per UNORDERED layer pair --
+ * nz(nz+1)/2 instead of nz^2, half the bytes again -- the other orientation uses the
+ * transpose (xz, yz negated) and H_i is multiplied by 1/dz_i at the end.
+ *   on = 2 (default): automatic.  fp32 plans with 8 <= nz <= 64 whose bank is in the mirror
+ *          storage use the block layout of the symmetric-matvec kernel (coupling_symv.cu):
+ *          every block is read from HBM once and applied to both of its layer pairs inside
+ *          one warp (info.mirror == 3), wherever that layout (nz padded to whole strips of
+ *          four layers) streams at least 30 % fewer bytes than the mirror bank.
+ *   on = 1: wherever the mirror storage is active: the block layout if fp32 and nz <= 64,
+ *          else the p <= q bank read through a pair table by the streaming kernel
+ *          (info.mirror == 2: saves memory, not time -- the second use of an entry is a
+ *          second read).
+ *   on = 0: never.
+ * hfft_update_dz rebuilds the whole bank in these modes.  Must be called before
  * hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
@@ -155,8 +181,14 @@ hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
  */
 hfft_status hfft_tensor_classes(int nz, const double *dz, int *cls_out, int *n_classes, int *toeplitz);
 
-/* Sizes the plan needs; valid after create / set_batch / set_dedup.  Errors: EINVAL. */
+/* Sizes the plan needs; valid after create and after every hfft_plan_set_* call (each of them may
+ * change the storage and with it the sizes).  Errors: EINVAL. */
 hfft_status hfft_plan_info(const hfft_plan *plan, hfft_info *info);
+
+/* The two sizes a caller who brings its own buffers needs, = info.bank_bytes and
+ * info.workspace_bytes.  0 for a NULL plan. */
+size_t hfft_bank_bytes(const hfft_plan *plan);
+size_t hfft_workspace_bytes(const hfft_plan *plan);
 
 /*
  * Optional: hand the plan caller-owned DEVICE buffers (e.g. torch tensors) of
@@ -189,17 +221,21 @@ hfft_status hfft_build_tensor(hfft_plan *plan, void *stream);
  *       PAPER.md:140, per-layer by reading A12), read during the call and passed
  *       by value to the kernels; NULL means 1.0 (m already holds M)
  *   h   DEVICE pointer, same shape and type as m, overwritten; units of Ms;
- *       must not alias m
+ *       the two arrays must not overlap, not even partially (EINVAL)
  * Only enqueues kernels on `stream`: no host synchronisation, no allocation,
- * safe to capture in a CUDA graph.  Errors: EINVAL, ESTATE (tensor not built),
- * ECUDA (launch failure).
+ * safe to capture in a CUDA graph.  Consecutive calls on one plan share its spectra:
+ * enqueue them on one stream (or order the streams yourself).  Errors: EINVAL,
+ * ESTATE (tensor not built; evaluations of hfft_demag_host_async outstanding -- call
+ * hfft_host_join first), ECUDA (launch failure).
  */
 hfft_status hfft_demag(hfft_plan *plan, const void *m, const double *Ms, void *h, void *stream);
 
 /*
  * Same evaluation with HOST buffers (pinned memory gives asynchronous copies):
- * copies m to a staging buffer inside the plan workspace, runs hfft_demag,
- * copies h back, all on `stream`.  Does not synchronise the stream.
+ * copies m to a staging buffer of the plan, runs hfft_demag, copies h back, all on
+ * `stream`.  Does not synchronise the stream.  The first host-path call of a plan
+ * allocates the staging buffers (four arrays of the size of m; freed by
+ * hfft_destroy).  Errors: as hfft_demag, ENOMEM.
  */
 hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *Ms, void *h_host,
                             void *stream);
@@ -218,7 +254,9 @@ hfft_status hfft_demag_host(hfft_plan *plan, const void *m_host, const double *M
  */
 hfft_status hfft_demag_host_async(hfft_plan *plan, const void *m_host, const double *Ms, void *h_host,
                                   void *stream);
-/* Makes `stream` wait for every hfft_demag_host_async issued so far (no host blocking). */
+/* Makes `stream` wait for every hfft_demag_host_async issued so far (no host blocking).  Until it is
+ * called, hfft_demag and hfft_demag_host on this plan return ESTATE: they would use the spectra the
+ * pipeline is still working on.  After it, issue them on `stream` (or on a stream ordered after it). */
 hfft_status hfft_host_join(hfft_plan *plan, void *stream);
 
 /*
@@ -279,7 +317,7 @@ hfft_status hfft_destroy(hfft_plan *plan);
  * to get the message of the last failing hfft_plan_create on this thread. */
 const char *hfft_last_error(const hfft_plan *plan);
 
-/* Library build identification, e.g. "hfft 0.1 sm_100a". */
+/* Library build identification, e.g. "hfft 0.3 sm_100a". */
 const char *hfft_version(void);
 
 #ifdef __cplusplus

@@ -24,7 +24,7 @@ MAX_NZ = 256
 
 # every symbol include/hfft.h declares
 EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror", "hfft_plan_set_recip",
-           "hfft_tensor_classes", "hfft_plan_info", "hfft_plan_set_buffers",
+           "hfft_tensor_classes", "hfft_plan_info", "hfft_bank_bytes", "hfft_workspace_bytes", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
@@ -67,6 +67,8 @@ def lib():
         L.hfft_plan_set_recip.argtypes = [vp, ctypes.c_int]
         L.hfft_tensor_classes.argtypes = [ctypes.c_int, dp, ip, ip, ip]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
+        L.hfft_bank_bytes.argtypes = [vp]
+        L.hfft_workspace_bytes.argtypes = [vp]
         L.hfft_plan_set_buffers.argtypes = [vp, vp, vp]
         L.hfft_build_tensor.argtypes = [vp, vp]
         L.hfft_demag.argtypes = [vp, vp, dp, vp, vp]
@@ -83,8 +85,10 @@ def lib():
         L.hfft_last_error.restype = ctypes.c_char_p
         L.hfft_version.restype = ctypes.c_char_p
         for name in EXPORTS:
-            if name not in ("hfft_last_error", "hfft_version"):
+            if name not in ("hfft_last_error", "hfft_version", "hfft_bank_bytes", "hfft_workspace_bytes"):
                 getattr(L, name).restype = ctypes.c_int
+        L.hfft_bank_bytes.restype = ctypes.c_size_t
+        L.hfft_workspace_bytes.restype = ctypes.c_size_t
         _lib = L
     return _lib
 
@@ -123,6 +127,14 @@ def plan_set_batch(plan, batch):
 def plan_set_dedup(plan, mode):
     """0 off, 1 automatic (default), 2 on, 3 z-FFT method (equal thicknesses; Eq.25)."""
     _check(lib().hfft_plan_set_dedup(plan, int(mode)), plan)
+
+
+def bank_bytes(plan) -> int:
+    return int(lib().hfft_bank_bytes(plan))
+
+
+def workspace_bytes(plan) -> int:
+    return int(lib().hfft_workspace_bytes(plan))
 
 
 def plan_set_mirror(plan, on):

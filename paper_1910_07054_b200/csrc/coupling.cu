@@ -444,17 +444,10 @@ static cudaError_t launch_coupling_class_t(const CouplingArgs& a, cudaStream_t s
     const size_t smem = coupling_class_smem_bytes(a.nz, a.n_classes, TOEP, sizeof(T));
     const int threads = 32 * ((a.nz + IPT - 1) / IPT);
     if (threads > (MINB == 2 ? 256 : ClassCfg<T, IPT>::MAXT)) return cudaErrorInvalidConfiguration;
-    static size_t smem_done = 0;
-    cudaError_t err;
-    if (smem > 48 * 1024 && smem > smem_done) {
-        err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        smem_done = smem;
-    }
-    int nb = 0;
-    err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
+    static PerDevice<int> cache;
+    int nb = 1;
+    cudaError_t err = ctas_per_sm_cached(kern, threads, smem, cache, nb);
     if (err != cudaSuccess) return err;
-    if (nb < 1) return cudaErrorInvalidConfiguration;
     long long grid = (long long)a.num_sms * nb;
     if (grid > a.n_tiles) grid = a.n_tiles;
     return launch_pdl(kern, dim3((unsigned)grid), dim3(threads), smem, st, (const T*)a.bank, (C*)a.spec, a.cls, a.nz, a.n_classes, a.batch,
@@ -493,18 +486,10 @@ static cudaError_t launch_coupling_batched_nz(const void* bank, void* spec, int 
     constexpr int THREADS = 32 * ((NZ + IPT - 1) / IPT);
     auto kern = coupling_batched_kernel<T, NZ, IPT, STAGES>;
     const size_t smem = (size_t)STAGES * 3 * NZ * 32 * sizeof(C);
-    static int occ_blocks = 0;
-    cudaError_t err;
-    if (occ_blocks == 0) {
-        if (smem > 48 * 1024) {
-            err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (err != cudaSuccess) return err;
-        }
-        int nb = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, THREADS, smem);
-        if (err != cudaSuccess) return err;
-        occ_blocks = nb < 1 ? 1 : nb;
-    }
+    static PerDevice<int> cache;
+    int occ_blocks = 1;
+    cudaError_t err = ctas_per_sm_cached(kern, THREADS, smem, cache, occ_blocks);
+    if (err != cudaSuccess) return err;
     long long grid = (long long)num_sms * occ_blocks;
     if (grid > n_tiles) grid = n_tiles;
     return launch_pdl(kern, dim3((unsigned)grid), dim3(THREADS), smem, st, (const T*)bank, (C*)spec, batch, n_tiles, ks);
@@ -542,21 +527,10 @@ static cudaError_t launch_coupling_k(const CouplingArgs& a, cudaStream_t st) {
     // so that enough bank loads are in flight (B200, 256 x 256 x 96 fp32: 3.92 -> 2.71 ms per evaluation)
     if (MIR && sizeof(T) == 4 && smem > 113 * 1024 && a.nz >= 32) warps = 32;
     const int threads = warps * 32;
-    static size_t smem_done = 0;
-    static int occ_threads = 0, occ_blocks = 0;
-    static size_t occ_smem = 0;
-    cudaError_t err;
-    if (smem > 48 * 1024 && smem > smem_done) {
-        err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (err != cudaSuccess) return err;
-        smem_done = smem;
-    }
-    if (occ_threads != threads || occ_smem != smem) {
-        int nb = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
-        if (err != cudaSuccess) return err;
-        occ_threads = threads; occ_smem = smem; occ_blocks = nb < 1 ? 1 : nb;
-    }
+    static PerDevice<int> cache;
+    int occ_blocks = 1;
+    cudaError_t err = ctas_per_sm_cached(kern, threads, smem, cache, occ_blocks);
+    if (err != cudaSuccess) return err;
     long long items = a.n_tiles * a.batch;
     long long grid = (long long)a.num_sms * occ_blocks;
     if (grid > items) grid = items;

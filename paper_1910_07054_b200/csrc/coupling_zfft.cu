@@ -267,19 +267,10 @@ static cudaError_t launch_zfft_l(const CouplingArgs& a, cudaStream_t st) {
     auto kern = coupling_zfft_kernel<T, L>;
     const size_t smem = ZOcc<T, L>::SMEM;
     const int threads = 32 * Z::TT;
-    static int occ = 0;
-    cudaError_t err;
-    if (occ == 0) {
-        if (smem > 48 * 1024) {
-            err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            if (err != cudaSuccess) return err;
-        }
-        int nb = 0;
-        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kern, threads, smem);
-        if (err != cudaSuccess) return err;
-        if (nb < 1) return cudaErrorInvalidConfiguration;
-        occ = nb;
-    }
+    static PerDevice<int> cache;
+    int occ = 1;
+    cudaError_t err = ctas_per_sm_cached(kern, threads, smem, cache, occ);
+    if (err != cudaSuccess) return err;
     const long long items = a.n_tiles * a.batch;
     long long grid = (long long)a.num_sms * occ;
     if (grid > items) grid = items;

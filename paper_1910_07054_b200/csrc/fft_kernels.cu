@@ -379,25 +379,8 @@ iffty_kernel(const HFFT_C* __restrict__ spec, HFFT_C* __restrict__ xhat, long lo
 // ------------------------------------------------------------------------------------------
 // host-side dispatch
 // ------------------------------------------------------------------------------------------
-// Per kernel instantiation: opt in to > 48 KB of dynamic shared memory and ask the runtime how
-// many CTAs fit an SM (cached for the last (threads, smem) pair; `Tag` makes one cache per case).
-struct LaunchCache { int threads = 0; size_t smem = 0, smem_opt = 0; int occ = 0; };
-template <typename K>
-static cudaError_t ctas_per_sm(K kernel, int threads, size_t smem, LaunchCache& lc, int& occ) {
-    cudaError_t e;
-    if (smem > 48 * 1024 && smem > lc.smem_opt) {
-        if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess) return e;
-        lc.smem_opt = smem;
-    }
-    if (lc.threads != threads || lc.smem != smem) {
-        int nb = 0;
-        if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, smem)) != cudaSuccess) return e;
-        lc.threads = threads; lc.smem = smem; lc.occ = nb < 1 ? 1 : nb;
-    }
-    occ = lc.occ;
-    return cudaSuccess;
-}
-
+// Per kernel instantiation: one PerDevice cache (hfft_internal.h) of the shared-memory opt-in and of the CTAs per SM
+// the runtime reports for (threads, smem), keyed by device.
 // persistent grid: `items` units of work in contiguous chunks of `per_cta`
 static void chunk_grid(long long items, int num_sms, int occ, unsigned& grid, int& per_cta) {
     long long g = (long long)num_sms * occ;
@@ -453,9 +436,9 @@ cudaError_t launch_fftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, in
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_X(log2nx, {
         auto kern = fftx_fwd_kernel<T, L, ZP>;
-        static LaunchCache lc;
+        static PerDevice<int> lc;
         int occ = 1;
-        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+        if ((err = ctas_per_sm_cached(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int bpc;
             chunk_grid(nblocks, num_sms, occ, grid, bpc);
             err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, in, (C*)xhat, log2rb, rows_per_plane, nz > 0 ? nz : 1, use_ms, ms,
@@ -479,9 +462,9 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
     if (sums) {
         HFFT_DISPATCH_X(log2nx, {
             auto kern = ifftx_kernel<T, L, true>;
-            static LaunchCache lc;
+            static PerDevice<int> lc;
             int occ = 1;
-            if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+            if ((err = ctas_per_sm_cached(kern, threads, smem, lc, occ)) == cudaSuccess) {
                 unsigned grid; int bpc;
                 chunk_grid(nblocks, num_sms, occ, grid, bpc);
                 err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
@@ -492,9 +475,9 @@ cudaError_t launch_ifftx(const void* xhat, T* out, int log2nx, int nplanes, int 
     }
     HFFT_DISPATCH_X(log2nx, {
         auto kern = ifftx_kernel<T, L, false>;
-        static LaunchCache lc;
+        static PerDevice<int> lc;
         int occ = 1;
-        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+        if ((err = ctas_per_sm_cached(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int bpc;
             chunk_grid(nblocks, num_sms, occ, grid, bpc);
             err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, out, log2rb, rows_per_plane, (const C*)tw,
@@ -519,9 +502,9 @@ cudaError_t launch_ffty_fwd(const void* xhat, void* spec, int nx, int log2N, int
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_Y(log2N, {
         auto kern = ffty_fwd_kernel<T, L, ZP>;
-        static LaunchCache lc;
+        static PerDevice<int> lc;
         int occ = 1;
-        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+        if ((err = ctas_per_sm_cached(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
             err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)xhat, (C*)spec, nrows, nx + 1, nz_rot, ks, (const C*)twt,
@@ -546,9 +529,9 @@ cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int np
     cudaError_t err = cudaErrorInvalidValue;
     HFFT_DISPATCH_Y(log2N, {
         auto kern = iffty_kernel<T, L>;
-        static LaunchCache lc;
+        static PerDevice<int> lc;
         int occ = 1;
-        if ((err = ctas_per_sm(kern, threads, smem, lc, occ)) == cudaSuccess) {
+        if ((err = ctas_per_sm_cached(kern, threads, smem, lc, occ)) == cudaSuccess) {
             unsigned grid; int gpc;
             chunk_grid(ngroups, num_sms, occ, grid, gpc);
             err = launch_pdl(kern, dim3(grid), dim3(threads), smem, st, (const C*)spec, (C*)xhat, nrows, nx + 1, nz_rot, ks, (const C*)twt,

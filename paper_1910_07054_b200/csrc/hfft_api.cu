@@ -25,8 +25,12 @@ struct hfft_plan {
     long long n_k = 0, n_k_padded = 0, n_tiles = 0;
     size_t elem = 4;
     size_t bank_bytes = 0, ws_bytes = 0;
-    size_t ws_xhat = 0, ws_spec = 0, ws_stage_m = 0, ws_stage_h = 0;   // offsets into the workspace
-    size_t ws_stage_m2 = 0, ws_stage_h2 = 0;         // second staging pair of the pipelined host path
+    size_t ws_xhat = 0, ws_spec = 0;                 // offsets into the workspace
+    // host paths: staging copies of m and h (two slots for the pipelined form), allocated on the first
+    // hfft_demag_host / hfft_demag_host_async call -- callers of the device path never pay for them
+    void* stage = nullptr;
+    size_t stage_bytes = 0;                          // of one buffer; layout m, h, m2, h2
+    bool pipe_unjoined = false;                      // hfft_demag_host_async issued since the last hfft_host_join
     // hfft_demag_host_async: copy-in, compute and copy-out streams, per staging slot events
     cudaStream_t s_h2d = nullptr, s_comp = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_user = nullptr, ev_h2d[2] = {nullptr, nullptr}, ev_comp[2] = {nullptr, nullptr},
@@ -241,16 +245,13 @@ static void plan_sizes(hfft_plan* p) {
     size_t o = 0;
     p->ws_xhat = o;    o += al(planes * (size_t)p->ny * (p->nx + 1) * 2 * e);
     p->ws_spec = o;    o += al(planes * (size_t)p->n_k_padded * 2 * e);
-    p->ws_stage_m = o; o += al(planes * (size_t)p->ny * p->nx * e);
-    p->ws_stage_h = o; o += al(planes * (size_t)p->ny * p->nx * e);
-    p->ws_stage_m2 = o; o += al(planes * (size_t)p->ny * p->nx * e);
-    p->ws_stage_h2 = o; o += al(planes * (size_t)p->ny * p->nx * e);
     p->ws_bytes = o;
+    p->stage_bytes = al(planes * (size_t)p->ny * p->nx * e);
 }
 
 extern "C" {
 
-const char* hfft_version(void) { return "hfft 0.2 sm_100a"; }
+const char* hfft_version(void) { return "hfft 0.3 sm_100a"; }
 
 const char* hfft_last_error(const hfft_plan* plan) { return plan ? plan->error.c_str() : g_create_error.c_str(); }
 
@@ -367,6 +368,10 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     return HFFT_OK;
 }
 
+size_t hfft_bank_bytes(const hfft_plan* plan) { return plan ? plan->bank_bytes : 0; }
+
+size_t hfft_workspace_bytes(const hfft_plan* plan) { return plan ? plan->ws_bytes : 0; }
+
 hfft_status hfft_plan_set_buffers(hfft_plan* plan, void* bank, void* workspace) {
     if (!plan) return HFFT_EINVAL;
     if (!bank || !workspace) return fail(plan, HFFT_EINVAL, "hfft_plan_set_buffers: NULL buffer");
@@ -394,17 +399,16 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     }
     // padded wavevectors of the spectra must hold finite values
     if ((e = cudaMemsetAsync(plan->ws, 0, plan->ws_bytes, st)) != cudaSuccess) return fail_cuda(plan, "cudaMemsetAsync", e);
-    if (!plan->tw_x64) {
-        if ((e = upload_twiddles(2 * plan->nx, false, &plan->tw_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if ((e = upload_thread_twiddles(plan->log2nx, false, &plan->twt_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if ((e = upload_thread_twiddles(plan->log2ny + 1, false, &plan->twt_y64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if (plan->prec == HFFT_F32) {
-            if ((e = upload_twiddles(2 * plan->nx, true, &plan->tw_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-            if ((e = upload_thread_twiddles(plan->log2nx, true, &plan->twt_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-            if ((e = upload_thread_twiddles(plan->log2ny + 1, true, &plan->twt_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        } else {
-            plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
-        }
+    // every table is guarded on its own: a build that failed half-way through the uploads is retried cleanly
+    if (!plan->tw_x64 && (e = upload_twiddles(2 * plan->nx, false, &plan->tw_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+    if (!plan->twt_x64 && (e = upload_thread_twiddles(plan->log2nx, false, &plan->twt_x64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+    if (!plan->twt_y64 && (e = upload_thread_twiddles(plan->log2ny + 1, false, &plan->twt_y64)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+    if (plan->prec == HFFT_F32) {
+        if (!plan->tw_x && (e = upload_twiddles(2 * plan->nx, true, &plan->tw_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if (!plan->twt_x && (e = upload_thread_twiddles(plan->log2nx, true, &plan->twt_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+        if (!plan->twt_y && (e = upload_thread_twiddles(plan->log2ny + 1, true, &plan->twt_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
+    } else {
+        plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
     }
     if (plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) return fail_cuda(plan, "1/dz table", e);
     if ((plan->dedup || plan->recip) && !plan->d_cls) {
@@ -498,14 +502,26 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
 
 extern "C" {
 
-hfft_status hfft_demag(hfft_plan* plan, const void* m, const double* Ms, void* h, void* stream) {
-    if (!plan) return HFFT_EINVAL;
+// argument checks of the device path; shared by hfft_demag and the host paths (which pass their staging buffers)
+static hfft_status demag_checked(hfft_plan* plan, const void* m, const double* Ms, void* h, void* stream) {
     if (!m || !h) return fail(plan, HFFT_EINVAL, "hfft_demag: NULL m or h");
     if (((size_t)m & 15) || ((size_t)h & 15)) return fail(plan, HFFT_EINVAL, "hfft_demag: m and h must be 16-byte aligned");
-    if (m == h) return fail(plan, HFFT_EINVAL, "hfft_demag: h must not alias m");
+    // S5 reads m (fused reductions) while it writes h: any overlap of the two ranges corrupts, not only m == h
+    const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
+    const size_t ma = (size_t)m, ha = (size_t)h;
+    if (ma < ha + bytes && ha < ma + bytes) return fail(plan, HFFT_EINVAL, "hfft_demag: h must not overlap m");
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag: call hfft_build_tensor first");
     cudaStream_t st = (cudaStream_t)stream;
     return plan->prec == HFFT_F32 ? demag_impl<float>(plan, m, Ms, h, st) : demag_impl<double>(plan, m, Ms, h, st);
+}
+
+static const char* kPipeBusy =
+    ": evaluations of hfft_demag_host_async are outstanding (they share the plan's spectra); call hfft_host_join first";
+
+hfft_status hfft_demag(hfft_plan* plan, const void* m, const double* Ms, void* h, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_demag") + kPipeBusy);
+    return demag_checked(plan, m, Ms, h, stream);
 }
 
 hfft_status hfft_plan_set_reduction(hfft_plan* plan, double* sums_device) {
@@ -525,11 +541,16 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
     if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    // the new thickness is committed only once the rebuild has gone through: a failure leaves dz as it was and the
+    // plan unbuilt (the bank may be half rewritten), never a bank that disagrees with dz
+    const double dz_old = plan->dz[k];
     plan->dz[k] = dz_new;
     BuildGeom g = make_geom(plan);
     void* scratch = nullptr;
-    if ((e = cudaMalloc(&scratch, build_scratch_bytes(g))) != cudaSuccess)
+    if ((e = cudaMalloc(&scratch, build_scratch_bytes(g))) != cudaSuccess) {
+        plan->dz[k] = dz_old;                                // nothing was touched: the plan stays built
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
+    }
     std::string msg;
     // reciprocity storage: every stored S_pq = dz_p R_pq of a changed pair is rebuilt from its representative (the
     // class tables select them), which here means the whole bank; and the 1 / dz table changes
@@ -537,8 +558,23 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
     if (e == cudaSuccess && plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) msg = "1/dz table";
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
-    if (e != cudaSuccess) { plan->built = false; return fail(plan, HFFT_ECUDA, "hfft_update_dz: " + msg); }
-    if (e2 != cudaSuccess) { plan->built = false; return fail_cuda(plan, "hfft_update_dz: cudaStreamSynchronize", e2); }
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        plan->dz[k] = dz_old;
+        plan->built = false;
+        if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_update_dz: " + msg);
+        return fail_cuda(plan, "hfft_update_dz: cudaStreamSynchronize", e2);
+    }
+    // the tensor classes of the new stack (hfft_plan_info.n_classes; the bank itself is not deduplicated here)
+    pair_classes(plan->nz, plan->dz.data(), plan->pair_class, plan->class_rep, plan->toeplitz);
+    plan->n_classes = (int)plan->class_rep.size();
+    return HFFT_OK;
+}
+
+// staging buffers of the host paths: m, h, and a second pair for the pipelined form
+static hfft_status stage_init(hfft_plan* p) {
+    if (p->stage) return HFFT_OK;
+    cudaError_t e = cudaMalloc(&p->stage, 4 * p->stage_bytes);
+    if (e != cudaSuccess) return fail(p, HFFT_ENOMEM, std::string("cudaMalloc(host-path staging): ") + cudaGetErrorString(e));
     return HFFT_OK;
 }
 
@@ -546,15 +582,19 @@ hfft_status hfft_demag_host(hfft_plan* plan, const void* m_host, const double* M
     if (!plan) return HFFT_EINVAL;
     if (!m_host || !h_host) return fail(plan, HFFT_EINVAL, "hfft_demag_host: NULL m or h");
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_demag_host: call hfft_build_tensor first");
+    if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_demag_host") + kPipeBusy);
     cudaStream_t st = (cudaStream_t)stream;
-    unsigned char* ws = static_cast<unsigned char*>(plan->ws);
-    const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
     cudaError_t e;
-    if ((e = cudaMemcpyAsync(ws + plan->ws_stage_m, m_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-        return fail_cuda(plan, "cudaMemcpyAsync(H2D)", e);
-    hfft_status s = hfft_demag(plan, ws + plan->ws_stage_m, Ms, ws + plan->ws_stage_h, stream);
+    if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    hfft_status s = stage_init(plan);
     if (s != HFFT_OK) return s;
-    if ((e = cudaMemcpyAsync(h_host, ws + plan->ws_stage_h, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
+    unsigned char* sg = static_cast<unsigned char*>(plan->stage);
+    const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
+    if ((e = cudaMemcpyAsync(sg, m_host, bytes, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+        return fail_cuda(plan, "cudaMemcpyAsync(H2D)", e);
+    s = demag_checked(plan, sg, Ms, sg + plan->stage_bytes, stream);
+    if (s != HFFT_OK) return s;
+    if ((e = cudaMemcpyAsync(h_host, sg + plan->stage_bytes, bytes, cudaMemcpyDeviceToHost, st)) != cudaSuccess)
         return fail_cuda(plan, "cudaMemcpyAsync(D2H)", e);
     return HFFT_OK;
 }
@@ -579,11 +619,13 @@ hfft_status hfft_demag_host_async(hfft_plan* plan, const void* m_host, const dou
     cudaError_t e;
     if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
     if ((e = pipe_init(plan)) != cudaSuccess) return fail_cuda(plan, "hfft_demag_host_async: streams / events", e);
-    unsigned char* ws = static_cast<unsigned char*>(plan->ws);
+    hfft_status s0 = stage_init(plan);
+    if (s0 != HFFT_OK) return s0;
+    unsigned char* sg = static_cast<unsigned char*>(plan->stage);
     const size_t bytes = (size_t)3 * plan->nz * plan->batch * plan->ny * plan->nx * plan->elem;
     const int slot = (int)(plan->pipe_calls & 1);
-    void* dm = ws + (slot ? plan->ws_stage_m2 : plan->ws_stage_m);
-    void* dh = ws + (slot ? plan->ws_stage_h2 : plan->ws_stage_h);
+    void* dm = sg + (size_t)(2 * slot) * plan->stage_bytes;
+    void* dh = sg + (size_t)(2 * slot + 1) * plan->stage_bytes;
     const bool reuse = plan->pipe_calls >= 2;        // the slot was used two calls ago
 #define HFFT_PIPE(call) if ((e = (call)) != cudaSuccess) return fail_cuda(plan, "hfft_demag_host_async: " #call, e)
     // copy-in: after everything the caller enqueued on `stream` so far, and after the evaluation that last read the slot
@@ -595,8 +637,9 @@ hfft_status hfft_demag_host_async(hfft_plan* plan, const void* m_host, const dou
     // evaluation: after its copy-in, and after the copy-out that last read the slot's h
     HFFT_PIPE(cudaStreamWaitEvent(plan->s_comp, plan->ev_h2d[slot], 0));
     if (reuse) HFFT_PIPE(cudaStreamWaitEvent(plan->s_comp, plan->ev_d2h[slot], 0));
-    hfft_status s = hfft_demag(plan, dm, Ms, dh, plan->s_comp);
+    hfft_status s = demag_checked(plan, dm, Ms, dh, plan->s_comp);
     if (s != HFFT_OK) return s;
+    plan->pipe_unjoined = true;
     HFFT_PIPE(cudaEventRecord(plan->ev_comp[slot], plan->s_comp));
     // copy-out
     HFFT_PIPE(cudaStreamWaitEvent(plan->s_d2h, plan->ev_comp[slot], 0));
@@ -613,6 +656,7 @@ hfft_status hfft_host_join(hfft_plan* plan, void* stream) {
     // copy-outs are serialised on one stream: the last one implies all the earlier ones
     HFFT_PIPE(cudaStreamWaitEvent((cudaStream_t)stream, plan->ev_d2h[(plan->pipe_calls - 1) & 1], 0));
 #undef HFFT_PIPE
+    plan->pipe_unjoined = false;
     return HFFT_OK;
 }
 
@@ -723,8 +767,9 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (!plan) return HFFT_OK;
     if (plan->own_bank && plan->bank) cudaFree(plan->bank);
     if (plan->own_ws && plan->ws) cudaFree(plan->ws);
-    if (plan->tw_x != plan->tw_x64) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
+    if (plan->prec == HFFT_F32) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
     cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
+    if (plan->stage) cudaFree(plan->stage);
     if (plan->s_h2d) {
         cudaStreamSynchronize(plan->s_h2d); cudaStreamSynchronize(plan->s_comp); cudaStreamSynchronize(plan->s_d2h);
         cudaStreamDestroy(plan->s_h2d); cudaStreamDestroy(plan->s_comp); cudaStreamDestroy(plan->s_d2h);
