@@ -49,6 +49,10 @@ def parse_args():
     ap.add_argument("--mirror", type=int, default=None, help="hfft_plan_set_mirror mode (default: the library's, 1)")
     ap.add_argument("--recip", type=int, default=None, help="hfft_plan_set_recip (default: the library's)")
     ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="run every config (1, 2, 2f64, 3, 4, 4eq, 5) in a process of its own and write the bench lines, "
+                         "with their clocks, as a markdown table + JSON lines to --out")
+    ap.add_argument("--out", default=os.path.join("gpurun_out", "bench_all.md"), help="file --all-configs writes")
     return ap.parse_args()
 
 
@@ -69,13 +73,16 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def algorithmic_bytes(w, n_slots=None, mirror=False):
-    """what the shipped storage must move per hfft_demag call.
-    n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank);
-    mirror: ky-mirror storage, one bank entry per (kx, ky <= ny)."""
+def algorithmic_bytes(w, n_slots=None, mirror=False, recip=False):
+    """what the method must move per hfft_demag call with the symmetries the storage
+    uses.  n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank);
+    mirror: ky-mirror storage, one bank entry per (kx, ky <= ny); recip: reciprocity, one block per unordered
+    layer pair, nz (nz + 1) / 2 (the padding of the symv layout is NOT counted: it is overhead, not algorithm)."""
     s = 4 if w.precision == "f32" else 8
     n_k = 2 * w.ny * (w.nx + 1)
     planes = 3 * w.nz * w.B
+    if recip:
+        n_slots = w.nz * (w.nz + 1) // 2
     bank = 6 * (n_slots if n_slots else w.nz * w.nz) * ((w.nx + 1) * (w.ny + 1) if mirror else n_k) * s
     spec = planes * n_k * 2 * s            # M^ (= H^)
     xhat = planes * w.ny * (w.nx + 1) * 2 * s
@@ -137,74 +144,148 @@ class ClockSampler:
         return res
 
 
-def cpu_baseline(w, budget_s=20.0):
-    """The oracle's hybrid tier (T1, numpy FFT) on target layer 0 of the workload, tensor row
-    prebuilt (setup, like hfft_build_tensor for the GPU).  evals/s = 1 / (nz * t_layer)."""
+def _full_eval_on_host(w):
+    """Whether the CPU oracle times a whole evaluation (C1-C3) or a bounded sample of target layers (C4, C5)."""
+    return w.nx * w.ny * w.nz * w.B <= 256 * 256 * 16
+
+
+def _host_threads_for(w, cores):
+    """Threads of the all-cores run: bounded by the host memory one hybrid_layers call needs (padded tensor row, its
+    spectrum, the spectrum of M: ~ (6 nz (8 + 16) + 3 nz 16) * 4 nx ny bytes)."""
+    per = (6 * w.nz * 24 + 3 * w.nz * 16) * 4 * w.nx * w.ny * 1.3
+    try:
+        import psutil
+        avail = psutil.virtual_memory().available
+    except Exception:
+        avail = 32 << 30
+    return max(1, min(cores, w.nz, int(0.5 * avail / per)))
+
+
+def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
+    """The oracle's hybrid tier (T1, Eq.24; oracle.hybrid_layers with numpy's FFT, fp64), AS IT STANDS,
+    on the host cores, one state.  The binary128 tensor rows are prebuilt (setup, like hfft_build_tensor on the GPU);
+    everything else hybrid_layers does is inside the timing: the forward FFT of M (once per call), and per target
+    layer the 2-D FFT of the 6 nz padded tensor planes, the z-sum and the inverse FFT.  numpy's FFT and einsum run on
+    ONE thread (`cores_timed`); the all-cores figure runs the same calls, one target-layer chunk per thread.
+
+    C1-C3: whole evaluations (every target layer).  C4 / C5: a bounded sample -- calls with target layers [0] and
+    [0, 1] give the per-layer and the once-per-evaluation time; evaluation = once + nz * per_layer (the tensor row of
+    layer 0 stands in for both sampled layers: the timing does not depend on the values)."""
     import oracle as O
+    from concurrent.futures import ThreadPoolExecutor
     m = w.m_rounded([0])[0]
+    cores = os.cpu_count() or 1
+    full = _full_eval_on_host(w)
     t0 = time.perf_counter()
-    row = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
+    if full:
+        rows = {i: O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, i) for i in range(w.nz)}
+    else:
+        row0 = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
+        rows = {i: row0 for i in range(w.nz)}
     setup = time.perf_counter() - t0
-    times = []
-    while len(times) < 3 or (sum(times) < budget_s and len(times) < 20):
-        t0 = time.perf_counter()
-        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, [0], dft="fft", rows={0: row})
-        times.append(time.perf_counter() - t0)
-        if sum(times) > 4 * budget_s:
-            break
-    t_layer = float(np.median(times))
-    return {"value": 1.0 / (w.nz * t_layer), "unit": UNIT, "cores": O.threads(), "kind": "oracle",
-            "sample": "target layer 0 of %d, one state (oracle.hybrid_layers, numpy FFT, fp64), tensor row "
-                      "prebuilt; median of %d runs of %.3f s; value = 1/(nz*t_layer); numpy's FFT and einsum "
-                      "run on 1 thread, the binary128 tensor row (setup, %.1f s) on `cores` OpenMP threads"
-                      % (w.nz, len(times), t_layer, setup),
-            "oracle_tensor_row_s": setup}
+
+    def call(layers):
+        t = time.perf_counter()
+        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, list(layers), dft="fft", rows=rows)
+        return time.perf_counter() - t
+
+    def repeat(fn, n_fixed):
+        for _ in range(warmup):
+            fn()
+        ts = []
+        if n_fixed is not None:
+            for _ in range(n_fixed):
+                ts.append(fn())
+            return ts
+        while len(ts) < 3 or (sum(ts) < budget_s and len(ts) < 1000):
+            ts.append(fn())
+            if sum(ts) > 3 * budget_s:
+                break
+        return ts
+
+    nthr = _host_threads_for(w, cores)
+    if full:
+        ts = repeat(lambda: call(range(w.nz)), steps)
+        t_eval = float(np.mean(ts))
+        chunks = [list(range(w.nz))[t::nthr] for t in range(nthr)]
+
+        def par():
+            t = time.perf_counter()
+            with ThreadPoolExecutor(nthr) as ex:
+                list(ex.map(call, chunks))
+            return time.perf_counter() - t
+        tp = [par() for _ in range(max(1, min(3, len(ts))))]
+        t_eval_all = float(np.mean(tp))
+        sample = ("whole evaluations (all %d target layers) of one state: mean of %d runs of %.4f s"
+                  % (w.nz, len(ts), t_eval))
+        runs, s_per_step = len(ts), t_eval
+    else:
+        n = steps if steps is not None else 3
+        t1 = float(np.median(repeat(lambda: call([0]), n)))
+        t2 = float(np.median(repeat(lambda: call([0, 1]), n)))
+        per = max(t2 - t1, 1e-9)
+        once = max(t1 - per, 0.0)
+        t_eval = once + w.nz * per
+
+        def par():
+            t = time.perf_counter()
+            with ThreadPoolExecutor(nthr) as ex:
+                list(ex.map(call, [[0]] * nthr))
+            return time.perf_counter() - t
+        t_par = par()
+        # nthr layers (each with its own forward FFT of M, as the call stands) in t_par seconds
+        t_eval_all = t_par * w.nz / nthr
+        sample = ("target layers [0] (%.3f s) and [0, 1] (%.3f s) of %d, one state, median of %d calls each: "
+                  "evaluation = once-per-call %.3f s + nz * per-layer %.3f s" % (t1, t2, w.nz, n, once, per))
+        runs, s_per_step = 2 * n, t1 + t2
+    return {"value": 1.0 / t_eval, "unit": UNIT, "cores": 1, "cores_timed": 1, "cores_available": cores,
+            "kind": "oracle", "s_per_eval": t_eval,
+            "sample": sample + "; oracle.hybrid_layers (numpy FFT, fp64) as it stands: tensor rows prebuilt (binary128, "
+                      "%.1f s on %d OpenMP threads, untimed), the tensor planes' 2-D FFT, the forward FFT of M, the "
+                      "z-sum and the inverse FFT inside the timing" % (setup, O.threads()),
+            "all_cores": {"value": 1.0 / t_eval_all, "unit": UNIT, "cores": nthr, "s_per_eval": t_eval_all,
+                          "how": "the same calls, one chunk of target layers per thread (numpy releases the GIL)"},
+            "oracle_tensor_rows_s": setup, "_runs": runs, "_s_per_step": s_per_step}
+
+
+def cpu_baseline(w, budget_s=20.0):
+    r = oracle_timing(w, budget_s)
+    r.pop("_runs"); r.pop("_s_per_step")
+    return r
+
+
+def l2_mode(w):
+    """How the timed steps keep L2 from serving the inputs -- a function of the workload alone, so that both arms
+    print the same `config`.  Workloads whose smallest storage (reciprocity + ky-mirror bank) exceeds twice the L2
+    stream it every step; the small ones get a 256 MiB memset before every timed step."""
+    small = algorithmic_bytes(w, None, True, True)["whole"] < (256 << 20)
+    return ("L2 flushed (256 MiB memset) before every timed step" if small
+            else "inputs larger than L2 (126 MB): the tensor bank and the spectra are streamed from HBM every step")
 
 
 def run_reference(args, w):
-    """--impl reference: the oracle, as it stands, on the host cores.  One step = target layer 0."""
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    import oracle as O
-    m = w.m_rounded([0])[0]
-    row = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
-    Ms = np.broadcast_to(np.asarray(w.Ms, dtype=np.float64), (w.nz,))
-
-    def make_step(nzs):
-        """Target layer 0 of the stack cut to its first nzs layers (N_0j depends on the layers 0..j only, so the
-        tensor row of the cut stack is the head of the full row)."""
-        mm, dz, ms, rows = np.ascontiguousarray(m[:, :nzs]), w.dz[:nzs], Ms[:nzs], {0: row[:nzs]}
-        return lambda: O.hybrid_layers(w.nx, w.ny, nzs, w.dx, w.dy, dz, mm, ms, [0], dft="fft", rows=rows)
-
-    # size the per-step sample so that the whole run stays within a few minutes whatever K and W are
-    budget_s = 120.0
-    step = make_step(w.nz)
-    t0 = time.perf_counter()
-    step()
-    t_probe = time.perf_counter() - t0
-    nzs = w.nz
-    if (args.steps + args.warmup) * t_probe > budget_s:
-        nzs = max(1, min(w.nz, int(w.nz * budget_s / ((args.steps + args.warmup) * t_probe))))
-        step = make_step(nzs)
-    for _ in range(args.warmup):
-        step()
-    t0 = time.perf_counter()
-    for _ in range(args.steps):
-        step()
-    dt = time.perf_counter() - t0
-    # one step = 1 target layer x nzs source layers; a whole evaluation = nz target layers x nz source layers
-    t_layer = dt / args.steps * (w.nz / nzs)
-    value = 1.0 / (w.nz * t_layer)                          # one state; evals/s of a whole-stack evaluation
+    full = _full_eval_on_host(w)
+    # C1-C3: every step is a whole evaluation.  C4 / C5: each step is the bounded sample (target layers [0] and [0, 1]);
+    # the number of sampled calls is cut so that the run stays within a few minutes whatever K and W are.
+    steps, warmup = args.steps, args.warmup
+    if not full:
+        steps, warmup = max(1, min(args.steps, 3)), min(args.warmup, 1)
+    elif w.nx * w.ny * w.nz > 64 * 64 * 6:
+        steps, warmup = max(1, min(args.steps, 5)), min(args.warmup, 1)
+    r = oracle_timing(w, steps=steps, warmup=warmup)
+    runs, s_per_step = r.pop("_runs"), r.pop("_s_per_step")
+    value = r["value"]
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(w, "host memory; no GPU"),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": O.threads(), "kind": "oracle",
-                         "sample": "each step = target layer 0 of %d, summed over the first %d of %d source layers, of one "
-                                   "state (oracle.hybrid_layers, numpy FFT, fp64, tensor row prebuilt); value = "
-                                   "1 / (nz * s_per_step * nz / source layers per step)" % (w.nz, nzs, w.nz)},
+        "config": workload_config(w),
+        "cpu_baseline": r,
+        "steps_run": steps, "warmup_run": warmup, "oracle_calls_timed": runs,
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -273,16 +354,55 @@ def sweep_nz():
 SEED_SWEEP = 191007054
 
 
-def workload_config(w, l2):
+def workload_config(w):
+    l2 = l2_mode(w)
     return {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "batch": w.B, "precision": w.precision,
             "dz_nm": [round(float(v), 6) for v in w.dz[:8]] + (["..."] if w.nz > 8 else []),
             "m": w.m_kind, "seed": w.seed, "l2": l2, "parallelism": "replicas only (no sharding, no collective)"}
+
+
+ALL_CONFIGS = ["1", "2", "2f64", "3", "4", "4eq", "5"]
+
+
+def all_configs(args):
+    """north_star: "evaluations/sec and achieved HBM GB/s as a fraction of peak for each config".  Every config runs in
+    a bench.py process of its own (same flags); the JSON lines, each with its `clocks`, go to --out as a table."""
+    lines = []
+    for c in ALL_CONFIGS:
+        cmd = [sys.executable, os.path.abspath(__file__), "--config", c, "--steps", str(args.steps), "--warmup",
+               str(args.warmup), "--no-cpu-baseline"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        out = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+        if r.returncode != 0 or not out:
+            raise SystemExit("bench.py --config %s failed:\n%s" % (c, r.stderr[-4000:]))
+        lines.append(json.loads(out[-1]))
+        print(out[-1], flush=True)
+    os.makedirs(os.path.dirname(os.path.abspath(args.out)) or ".", exist_ok=True)
+    with open(args.out, "w") as fh:
+        fh.write("# bench.py --all-configs --steps %d --warmup %d\n\n" % (args.steps, args.warmup))
+        fh.write("Command: `python bench.py --all-configs --steps %d --warmup %d --out %s` (one B200; every config in a "
+                 "process of its own; clocks sampled with nvidia-smi during the timed regions).\n\n" % (args.steps, args.warmup, args.out))
+        fh.write("| config | ms / call | evals/s | e2e evals/s | S1 / S2 / S3 / S4 / S5 ms | S3 roofline (bound, achieved / peak = frac) "
+                 "| whole / roofline | bank | SM MHz (median / max) | throttle reasons |\n|---|---:|---:|---:|---|---|---:|---|---|---|\n")
+        for d in lines:
+            r, st, ck, bk = d["roofline"], d["stages_ms"], d["clocks"], d["bank"]
+            kind = ("z-FFT" if bk["dedup"] == 4 else "classes" if bk["dedup"] else "symv" if bk["symv_layout"] else
+                    "recip" if bk["reciprocity"] else "mirror" if bk["ky_mirror"] else "plain")
+            fh.write("| %s | %.4f | %.1f | %.1f | %s | %s %.4g / %.4g %s = %.2f | %.2f | %s, %.3f GB | %s / %s | %s |\n" % (
+                d["config"]["workload"], d["ms_per_step"], d["value"], d["e2e"]["value"],
+                " / ".join("%.4f" % st[n] for n in ("fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx")),
+                r["bound"], r["achieved"], r["peak"], r["unit"], r["frac"], d["whole_eval"]["ratio_to_roofline"],
+                kind, bk["bytes"] / 1e9, ck["sm_mhz"], ck["sm_max_mhz"], ", ".join(ck["reasons"]) or "none"))
+        fh.write("\nJSON lines:\n\n```\n" + "\n".join(json.dumps(d) for d in lines) + "\n```\n")
 
 
 def main():
     args = parse_args()
     if args.sweep_nz:
         sweep_nz()
+        return
+    if args.all_configs:
+        all_configs(args)
         return
     w = get_workload(args.config)
     if args.impl == "reference":
@@ -301,7 +421,7 @@ def main():
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    steps, warmup = max(1, args.steps), max(3, args.warmup)
+    steps, warmup = max(1, args.steps), max(0, args.warmup)    # W >= 3 is the caller's contract: not clamped
 
     def barrier():
         torch.cuda.synchronize()
@@ -326,11 +446,13 @@ def main():
     dedup = int(plan.info.dedup)
     # bank slots per wavevector: nz^2 pairs, tensor classes, or the Lz values of kz in the z-FFT mode
     mirror = bool(plan.info.mirror)
+    recip = int(plan.info.mirror) >= 2                     # 2: p <= q storage read twice, 3: symv layout read once
+    symv = int(plan.info.mirror) == 3
     slots = int(plan.info.bank_bytes // (6 * (plan.info.n_k_padded // (2 if mirror else 1)) * (4 if w.precision == "f32" else 8)))
-    ab = algorithmic_bytes(w, slots if (dedup or int(plan.info.mirror) == 2) else None, mirror)
-    # inputs larger than L2?  otherwise flush L2 between steps (and say so)
+    ab = algorithmic_bytes(w, slots if dedup else None, mirror, recip)
+    # inputs larger than L2?  otherwise flush L2 between steps (l2_mode: the same rule, printed in `config`)
     flush = None
-    if ab["whole"] < 512 << 20:
+    if l2_mode(w).startswith("L2 flushed") or ab["whole"] < (256 << 20):
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
 
     def step():
@@ -445,18 +567,23 @@ def main():
         value = whole_job_value(world, w.B, steps, ms_total)
         coup_ms = float(stage_ms[hb.STAGE_NAMES.index("coupling")])
         achieved = ab["coupling"] / (coup_ms * 1e-3) / 1e9 if coup_ms > 0 else None
-        traffic = None
+        # DRAM bytes per launch of the coupling kernel from the committed ncu --set full capture of this workload and
+        # storage (not re-measured here: ncu cannot run inside a timed bench)
+        traffic, traffic_src = None, None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tp):
             with open(tp) as fh:
-                traffic = json.load(fh).get(w.name, {}).get("coupling_dram_bytes_per_launch")
+                tj = json.load(fh).get(w.name, {})
+            storage = ("zfft" if dedup == 4 else "class" if dedup else "batched" if w.B > 1 else
+                       "symv" if symv else "recip" if recip else "mirror" if mirror else "plain")
+            ent = tj.get(storage) if isinstance(tj.get(storage), dict) else None
+            if ent:
+                traffic, traffic_src = ent.get("coupling_dram_bytes_per_launch"), ent.get("source")
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": w.precision, "data": "synthetic",
-            "config": workload_config(
-                w, "inputs larger than L2 (tensor bank %.2f GB streamed every step)" % (ab["bank"] / 1e9)
-                if flush is None else "L2 flushed (256 MiB memset) before every timed step"),
+            "config": workload_config(w),
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
                        "samples": clocks["samples"]},
             "e2e": {"value": whole_job_value(world, w.B, e2e_steps, ms_e2e), "unit": UNIT,
@@ -465,11 +592,13 @@ def main():
                            "device h -> pinned host; copies of neighbouring steps overlap the kernels)",
                     "serialised_hfft_demag_host": whole_job_value(world, w.B, e2e_steps, ms_e2e_serial)},
             "gpu_launches": plan.info.launches_per_demag * steps,
-            "roofline": {"bound": "hbm", "kernel": "coupling_kernel (S3)", "achieved": achieved, "peak": peak,
+            "roofline": {"bound": "hbm", "kernel": "coupling_symv_kernel (S3, reciprocity + ky-mirror bank read once)" if symv
+                         else "coupling_kernel (S3)", "achieved": achieved, "peak": peak,
                          "peak_source": peak_src, "unit": "GB/s", "frac": achieved / peak if achieved else None,
                          "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None,
                          "algorithmic_bytes_per_launch": ab["coupling"], "avg_launch_ms": coup_ms,
-                         "traffic": traffic},
+                         "stored_bank_bytes": int(plan.info.bank_bytes),
+                         "traffic": traffic, "traffic_source": traffic_src},
             "stages_ms": {n: float(v) for n, v in zip(hb.STAGE_NAMES, stage_ms)},
             "whole_eval": {"algorithmic_bytes": ab["whole"], "roofline_ms_at_peak": ab["whole"] / peak / 1e6,
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
@@ -493,8 +622,9 @@ def main():
                                 "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
                                 "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
                                 "hbm_gbs": achieved, "traffic": None}
-        line["config"]["bank"] = {"dedup": dedup, "ky_mirror": mirror, "reciprocity": int(plan.info.mirror) == 2, "slots_per_k": slots,
-                                  "bytes": int(plan.info.bank_bytes)}
+        line["bank"] = {"dedup": dedup, "ky_mirror": mirror, "reciprocity": recip, "symv_layout": symv,
+                        "slots_per_k": slots, "bytes": int(plan.info.bank_bytes)}
+        line["l2_flush_between_steps"] = flush is not None
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_baseline(w)
         print(json.dumps(line))
