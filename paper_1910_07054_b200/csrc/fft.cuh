@@ -27,14 +27,6 @@ namespace hfft {
 // visible (no-op when the kernel was not launched as a dependent)
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
-// Mirror layout of a spectrum row (hfft_plan_set_mirror): the tensor spectra are even (xx, yy, zz, xz) or
-// odd (xy, yz) in ky, so ky and 2ny - ky can share one bank entry.  A row then has N + 2 slots: ky <= N/2 sits at
-// 2 ky, its mirror N - ky at 2 ky + 1; ky = 0 and ky = N/2 are their own mirrors, their odd slots (1 and N + 1) are
-// dummies that hold zeros (never written by S2, H^ = N^ 0 = 0 written by S3, ignored by S4).
-__device__ __forceinline__ int ypos(int ky, int N, int mirror) {
-    return mirror ? (ky <= N / 2 ? 2 * ky : 2 * (N - ky) + 1) : ky;
-}
-
 template <typename T> struct cplx_of;
 template <> struct cplx_of<float> { typedef float2 type; };
 template <> struct cplx_of<double> { typedef double2 type; };

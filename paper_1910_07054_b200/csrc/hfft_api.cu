@@ -42,7 +42,6 @@ struct hfft_plan {
     // length-2ny row transforms (fft.cuh).  *64: fp64 copies for the setup (aliases for an fp64 plan).
     void *tw_x = nullptr, *twt_x = nullptr, *twt_y = nullptr;
     void *tw_x64 = nullptr, *twt_x64 = nullptr, *twt_y64 = nullptr;
-    void *tw_y = nullptr, *twh_x = nullptr, *twh_y = nullptr;   // experiment: fft_hot.cu
     double* sums = nullptr;                          // hfft_plan_set_reduction: [B][3][nz][2] on device
     // tensor classes (hfft_plan_set_dedup): pair -> class, class -> representative pair i*nz+j
     int dedup_mode = 1;                              // 0 off, 1 auto, 2 on, 3 z-FFT (Eq.25)
@@ -131,25 +130,6 @@ static void thread_twiddle_table(int log2N, std::vector<double>& re, std::vector
     if (re.empty()) { re.push_back(1.0); im.push_back(0.0); }   // single-stage transforms read nothing
 }
 
-static void sub_twiddle_table(int log2M, int log2Rmax, std::vector<double>& re, std::vector<double>& im) {
-    const int M = 1 << log2M, log2R = log2M < log2Rmax ? log2M : log2Rmax, R = 1 << log2R, TPR = M / R;
-    std::vector<double> tr, ti;
-    twiddle_table(M, tr, ti);
-    re.clear(); im.clear();
-    for (int lns = log2R; lns < log2M;) {
-        const int lr = (log2M - lns >= log2R) ? log2R : log2M - lns;
-        const int rad = 1 << lr, NS = 1 << lns;
-        for (int t = 1; t < rad; ++t)
-            for (int j = 0; j < TPR; ++j) {
-                const long long k = rad == R ? (j & (NS - 1)) : j;
-                const long long idx = (t * k * (M >> (lns + lr))) % M;
-                re.push_back(tr[idx]); im.push_back(ti[idx]);
-            }
-        lns += lr;
-    }
-    if (re.empty()) { re.push_back(1.0); im.push_back(0.0); }
-}
-
 static cudaError_t upload_complex(const std::vector<double>& re, const std::vector<double>& im, bool f32, void** out) {
     const size_t n = re.size();
     cudaError_t e;
@@ -172,12 +152,6 @@ static cudaError_t upload_twiddles(int N, bool f32, void** out) {
 static cudaError_t upload_thread_twiddles(int log2N, bool f32, void** out) {
     std::vector<double> re, im;
     thread_twiddle_table(log2N, re, im);
-    return upload_complex(re, im, f32, out);
-}
-
-static cudaError_t upload_sub_twiddles(int log2M, bool f32, void** out) {
-    std::vector<double> re, im;
-    sub_twiddle_table(log2M, f32 ? 4 : 3, re, im);
     return upload_complex(re, im, f32, out);
 }
 
@@ -436,12 +410,6 @@ hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     } else {
         plan->tw_x = plan->tw_x64; plan->twt_x = plan->twt_x64; plan->twt_y = plan->twt_y64;
     }
-    {
-        const bool f32 = plan->prec == HFFT_F32;
-        if (!plan->tw_y && (e = upload_twiddles(2 * plan->ny, f32, &plan->tw_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if (!plan->twh_x && (e = upload_sub_twiddles(plan->log2nx - 1, f32, &plan->twh_x)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-        if (!plan->twh_y && (e = upload_sub_twiddles(plan->log2ny, f32, &plan->twh_y)) != cudaSuccess) return fail_cuda(plan, "twiddles", e);
-    }
     if (plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) return fail_cuda(plan, "1/dz table", e);
     if ((plan->dedup || plan->recip) && !plan->d_cls) {
         const std::vector<int>& tab = plan->recip ? plan->recip_cls : plan->pair_class;
@@ -506,23 +474,24 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
 #define STAGE(idx, call)                                                            \
     if (ev && (e = cudaEventRecord(ev[idx], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e); \
     if ((e = (call)) != cudaSuccess) return fail_cuda(p, #call, e);
-    STAGE(0, (launch_hfftx_fwd<T>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, p->twh_x, p->num_sms, st)))
+    STAGE(0, (launch_fftx_fwd<T, true>((const T*)m, xhat, p->log2nx, planes, p->ny, p->nz, Ms, p->tw_x, p->twt_x,
+                                       p->num_sms, st)))
     // the z components are rotated by i on the k side (real form R6) except in the z-FFT mode
     const int nz_rot = p->zfft ? 0 : p->nz;
-    STAGE(1, (launch_hffty_fwd<T>(xhat, spec, p->nx, p->log2ny, planes, nz_rot, p->n_k_padded, p->tw_y, p->twh_y,
-                                  p->num_sms, st, p->mirror ? 1 : 0)))
+    STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y,
+                                       p->num_sms, st, p->mirror ? 1 : 0)))
     CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
                     p->recip ? (int)p->recip_rep.size() : (p->dedup ? p->n_classes : p->nz * p->nz),
                     (p->dedup || p->recip) ? p->d_cls : nullptr, p->class_kernel, p->toeplitz, p->num_sms};
     ca.recip = p->recip; ca.inv_dz = p->d_invdz; ca.symv = p->symv;
     ca.zfft = p->zfft; ca.log2lz = p->log2lz; ca.twz = p->d_twz; ca.mirror = p->mirror;
     STAGE(2, (launch_coupling<T>(ca, st)))
-    STAGE(3, (launch_hiffty<T>(spec, xhat, p->nx, p->log2ny, planes, nz_rot, p->n_k_padded, p->tw_y, p->twh_y, p->num_sms,
-                               st, p->mirror ? 1 : 0)))
+    STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st,
+                              p->mirror ? 1 : 0)))
     if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
         return fail_cuda(p, "cudaMemsetAsync(sums)", e);
-    STAGE(4, (launch_hifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twh_x, p->num_sms, (const T*)m,
-                               p->sums, st)))
+    STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, (const T*)m,
+                              p->sums, st)))
 #undef STAGE
     if (ev) {
         if ((e = cudaEventRecord(ev[HFFT_NUM_STAGES], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);
@@ -800,7 +769,6 @@ hfft_status hfft_destroy(hfft_plan* plan) {
     if (plan->own_ws && plan->ws) cudaFree(plan->ws);
     if (plan->prec == HFFT_F32) { cudaFree(plan->tw_x); cudaFree(plan->twt_x); cudaFree(plan->twt_y); }
     cudaFree(plan->tw_x64); cudaFree(plan->twt_x64); cudaFree(plan->twt_y64);
-    cudaFree(plan->tw_y); cudaFree(plan->twh_x); cudaFree(plan->twh_y);
     if (plan->stage) cudaFree(plan->stage);
     if (plan->s_h2d) {
         cudaStreamSynchronize(plan->s_h2d); cudaStreamSynchronize(plan->s_comp); cudaStreamSynchronize(plan->s_d2h);

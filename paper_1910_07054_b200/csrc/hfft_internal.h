@@ -102,20 +102,6 @@ template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
                          const void* twt_N, int num_sms, cudaStream_t st, int mirror = 0);
 
-// ---- fft_hot.cu: the hot-path transforms (two half-length sub-transforms per padded / cropped row; subfft.cuh) ----
-template <typename T>
-cudaError_t launch_hfftx_fwd(const T* in, void* xhat, int log2nx, int nplanes, int rows_per_plane, int nz,
-                             const double* ms_host, const void* tw2nx, const void* twh_x, int num_sms, cudaStream_t st);
-template <typename T>
-cudaError_t launch_hifftx(const void* xhat, T* out, int log2nx, int nplanes, int rows_per_plane, const void* tw2nx,
-                          const void* twh_x, int num_sms, const T* m, double* sums, cudaStream_t st);
-template <typename T>
-cudaError_t launch_hffty_fwd(const void* xhat, void* spec, int nx, int log2ny, int nplanes, int nz_rot, long long ks,
-                             const void* tw2ny, const void* twh_y, int num_sms, cudaStream_t st, int mirror);
-template <typename T>
-cudaError_t launch_hiffty(const void* spec, void* xhat, int nx, int log2ny, int nplanes, int nz_rot, long long ks,
-                          const void* tw2ny, const void* twh_y, int num_sms, cudaStream_t st, int mirror);
-
 // ---- coupling.cu ----
 // H^ = bank * M^ in place on the k side.  bank layout [tile][class][6][tile_k]; class = i*nz+j (cls == nullptr)
 // or cls[i*nz+j] (deduplicated bank, device table).
