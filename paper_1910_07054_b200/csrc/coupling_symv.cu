@@ -12,8 +12,8 @@
 // that lane by warp shuffle -- no shared-memory traffic for M^ / H^ in the loop and no barrier: the warps of a CTA run
 // independently.  The diagonal and the half block need no exchange beyond that (symv_layout.h).
 //
-// Bank stream.  The unit's stream is contiguous (NC couples of 768 B).  Each warp runs its own NS-deep ring of 1.5 KB
-// stages in shared memory, filled by bulk asynchronous copies (cp.async.bulk, the TMA engine; SASS UBLKCP) that signal an
+// Bank stream.  The unit's stream is contiguous (NC couples of 768 B).  Each warp runs its own ring of NS stages of four
+// couples (3 KB; the last stage of a unit is a single couple) in shared memory, filled by bulk asynchronous copies (cp.async.bulk, the TMA engine; SASS UBLKCP) that signal an
 // mbarrier per stage, with an L2 evict-first policy (every bank byte is used once); lane 0 re-arms a stage as soon as
 // the warp has consumed it, across unit boundaries, so the stream never drains between tiles.  The 16 strip-lanes read a
 // stage with 128-bit shared loads (the two mirror-slot lanes of a strip read the same address: broadcast).
@@ -76,14 +76,20 @@ struct Couple {
 #pragma unroll
         for (int j = 0; j < 3; ++j) v[j] = lds128(addr + 256 * j);
     }
-    // pair h (0 / 1) as a0..a5 = (xx, yy, zz, xy, xz, yz); sm flips xy, yz (mirror slot), tm flips xz, yz (transpose)
+    // pair h (0 / 1) as a0..a5 = (xx, yy, zz, xy, xz, yz); tm flips xz, yz (transpose).  The sign change of xy, yz on the
+    // mirror wavevector 2ny - ky is NOT applied here: A' = D A D with D = diag(1, -1, 1), so the odd-slot lanes work on
+    // D M^ and produce D H^ with the stored block as it is (the y components are negated once per tile, on the way
+    // in and on the way out, instead of two sign flips per block).
     template <int H>
-    __device__ __forceinline__ void get(float (&a)[6], uint32_t sm, uint32_t tm) const {
+    __device__ __forceinline__ void get(float (&a)[6]) const {
         if (H == 0) { a[0] = v[0].x; a[1] = v[0].y; a[2] = v[0].z; a[3] = v[0].w; a[4] = v[1].x; a[5] = v[1].y; }
         else        { a[0] = v[1].z; a[1] = v[1].w; a[2] = v[2].x; a[3] = v[2].y; a[4] = v[2].z; a[5] = v[2].w; }
-        a[3] = fxor(a[3], sm);
+    }
+    template <int H>
+    __device__ __forceinline__ void get(float (&a)[6], uint32_t tm) const {
+        get<H>(a);
         a[4] = fxor(a[4], tm);
-        a[5] = fxor(a[5], sm ^ tm);
+        a[5] = fxor(a[5], tm);
     }
 };
 
@@ -108,7 +114,7 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
                      int nz, int batch, long long n_tiles, long long ks) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const SymvGeom G = symv_geom(nz);
-    const int W = G.W, LW = G.LW, EPW = G.EPW, SPE = G.SPE;
+    const int W = G.W, LW = G.LW, EPW = G.EPW;
     const int TE = NWARP * EPW;                              // entries per CTA tile; 2 TE spectrum slots per row
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int s = lane & 1, g = lane >> 1;                   // mirror slot, strip-lane
@@ -116,9 +122,10 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     const bool act = w < W;
     const uint32_t smask = s ? 0x80000000u : 0u;             // odd slot = mirror wavevector 2ny - ky: xy, yz change sign
 
+    constexpr uint32_t STAGE = 4 * kSymvCoupleBytes;          // bytes of a full stage
     const uint32_t bars = smem_u32(smem_raw) + warp * (NS * 8);
-    const uint32_t ring = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + warp * (NS * kSymvStageBytes);
-    const uint32_t tile = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + NWARP * NS * kSymvStageBytes;
+    const uint32_t ring = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + warp * (NS * STAGE);
+    const uint32_t tile = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + NWARP * NS * STAGE;
     const uint32_t lane_off = (uint32_t)g * 16;
 
     // ---- this lane's slots in the M^ / H^ tile: row (c nz + 4 w + r), 16-byte chunk el ^ swizzle(w), half s ----
@@ -128,26 +135,29 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     const uint32_t row_bytes = (uint32_t)TE * 16;
 
     // ---- bank ring: producer state (uniform over the warp; lane 0 issues) ----
-    // this CTA's tiles: blockIdx.x, blockIdx.x + gridDim.x, ...; every tile is streamed once per state of the batch
+    // this CTA's tiles: blockIdx.x, blockIdx.x + gridDim.x, ...; every tile is streamed once per state of the batch.
+    // The bookkeeping is kept to a pointer, two counters and one comparison per stage: it runs once per 144 FFMA2.
     const int my_tiles = (int)((n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x);
-    const long long unit_bytes = (long long)G.NC * kSymvCoupleBytes;
-    const long long tile_stride = (long long)gridDim.x * NWARP * unit_bytes;
-    const char* p_unit = reinterpret_cast<const char*>(bank) + ((long long)blockIdx.x * NWARP + warp) * unit_bytes;
-    int p_tiles = my_tiles, p_b = 0, p_stage = 0;
-    uint32_t pg = 0, cg = 0;
+    const uint32_t unit_bytes = (uint32_t)G.NC * kSymvCoupleBytes;
+    const int stages_per_unit = (G.NC + 3) >> 2;              // NC = 1 (mod 4): the last stage is one couple
+    const long long tile_skip = (long long)gridDim.x * NWARP * unit_bytes - unit_bytes;
+    const char* p_ptr = reinterpret_cast<const char*>(bank) + ((long long)blockIdx.x * NWARP + warp) * unit_bytes;
+    int p_tiles = my_tiles, p_rep = batch, p_left = stages_per_unit;
+    uint32_t cg = 0;
     const uint64_t pol = evict_first_policy();
-    auto produce = [&]() {
+    // fetch the next stage of the stream into ring slot `slot`
+    auto produce = [&](uint32_t slot) {
         if (p_tiles > 0) {
+            const uint32_t bytes = p_left == 1 ? (uint32_t)kSymvCoupleBytes : STAGE;
             if (lane == 0) {
-                const uint32_t bytes = p_stage == SPE - 1 ? kSymvCoupleBytes : kSymvStageBytes;
-                const uint32_t slot = pg & (NS - 1);
                 mbar_expect_tx(bars + slot * 8, bytes);
-                bulk_g2s(ring + slot * kSymvStageBytes, p_unit + p_stage * kSymvStageBytes, bytes, bars + slot * 8, pol);
+                bulk_g2s(ring + slot * STAGE, p_ptr, bytes, bars + slot * 8, pol);
             }
-            ++pg;
-            if (++p_stage == SPE) {
-                p_stage = 0;
-                if (++p_b == batch) { p_b = 0; --p_tiles; p_unit += tile_stride; }
+            p_ptr += bytes;
+            if (--p_left == 0) {
+                p_left = stages_per_unit;
+                if (--p_rep == 0) { p_rep = batch; --p_tiles; p_ptr += tile_skip; }
+                else p_ptr -= unit_bytes;
             }
         }
     };
@@ -155,13 +165,14 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     auto acquire = [&]() -> uint32_t {
         const uint32_t slot = cg & (NS - 1);
         mbar_wait(bars + slot * 8, (cg / NS) & 1);
-        return ring + slot * kSymvStageBytes + lane_off;
+        return ring + slot * STAGE + lane_off;
     };
     // the warp is done with the stage: refill it
     auto release = [&]() {
+        const uint32_t slot = cg & (NS - 1);
         ++cg;
         __syncwarp();
-        produce();
+        produce(slot);
     };
 
     if (lane == 0) {
@@ -171,7 +182,7 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     }
     __syncwarp();
 #pragma unroll
-    for (int i = 0; i < NS; ++i) produce();                  // the bank does not depend on the previous kernel
+    for (int i = 0; i < NS; ++i) produce(i);                 // the bank does not depend on the previous kernel
 
     pdl_wait();                                              // M^ comes from the previous kernel (S2)
 
@@ -204,6 +215,7 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
                 mp[r][c] = live ? lds<float2>(my_slot + (uint32_t)(c * nz + layer) * row_bytes) : make_float2(0.f, 0.f);
                 hp[r][c] = make_float2(0.f, 0.f);
             }
+            mp[r][1] = make_float2(fxor(mp[r][1].x, smask), fxor(mp[r][1].y, smask));      // D M^ on the mirror slot
         }
 
         // ---- full blocks T = 1 .. nfull: strip w against strip (w + T) mod W ----
@@ -214,22 +226,26 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
             const int src_m = act ? (lane & ~(2 * LW - 2)) | (wp << 1) : lane;     // owner of the block's source layers
             const int src_c = act ? (lane & ~(2 * LW - 2)) | (wm << 1) : lane;     // strip whose block targets my layers
 #pragma unroll
-            for (int cc = 0; cc < 4; ++cc) {
-                float2 mq[3], cq[3];
-#pragma unroll
-                for (int c = 0; c < 3; ++c) { mq[c] = shfl2(mp[cc][c], src_m); cq[c] = make_float2(0.f, 0.f); }
+            for (int c2 = 0; c2 < 2; ++c2) {                 // one stage = two columns of the block
                 const uint32_t st = acquire();
-                Couple k0, k1;
-                k0.load(st);
-                k1.load(st + kSymvCoupleBytes);
-                float a[6];
-                k0.get<0>(a, smask, 0u); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
-                k0.get<1>(a, smask, 0u); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
-                k1.get<0>(a, smask, 0u); mv(hp[2], a, mq); mvT(cq, a, mp[2]);
-                k1.get<1>(a, smask, 0u); mv(hp[3], a, mq); mvT(cq, a, mp[3]);
-                release();
 #pragma unroll
-                for (int c = 0; c < 3; ++c) hp[cc][c] = cadd(hp[cc][c], shfl2(cq[c], src_c));
+                for (int hh = 0; hh < 2; ++hh) {
+                    const int cc = 2 * c2 + hh;
+                    float2 mq[3], cq[3];
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) { mq[c] = shfl2(mp[cc][c], src_m); cq[c] = make_float2(0.f, 0.f); }
+                    Couple k0, k1;
+                    k0.load(st + hh * 2 * kSymvCoupleBytes);
+                    k1.load(st + hh * 2 * kSymvCoupleBytes + kSymvCoupleBytes);
+                    float a[6];
+                    k0.get<0>(a); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
+                    k0.get<1>(a); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
+                    k1.get<0>(a); mv(hp[2], a, mq); mvT(cq, a, mp[2]);
+                    k1.get<1>(a); mv(hp[3], a, mq); mvT(cq, a, mp[3]);
+                    if (hh == 1) release();
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) hp[cc][c] = cadd(hp[cc][c], shfl2(cq[c], src_c));
+                }
             }
         }
 
@@ -249,43 +265,41 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
             // column 1
 #pragma unroll
             for (int c = 0; c < 3; ++c) { mq[c] = shfl2(mp[1][c], src); cq[c] = make_float2(0.f, 0.f); }
-            k0.get<0>(a, smask, 0u); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
+            k0.get<0>(a); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
 #pragma unroll
             for (int c = 0; c < 3; ++c) hp[1][c] = cadd(hp[1][c], shfl2(cq[c], src));
             // column 2
 #pragma unroll
             for (int c = 0; c < 3; ++c) { mq[c] = shfl2(mp[2][c], src); cq[c] = make_float2(0.f, 0.f); }
-            k0.get<1>(a, smask, 0u); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
-            k1.get<0>(a, smask, 0u); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
+            k0.get<1>(a); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
+            k1.get<0>(a); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
 #pragma unroll
             for (int c = 0; c < 3; ++c) hp[2][c] = cadd(hp[2][c], shfl2(cq[c], src));
             // column 3
 #pragma unroll
             for (int c = 0; c < 3; ++c) { mq[c] = shfl2(mp[3][c], src); cq[c] = make_float2(0.f, 0.f); }
-            k1.get<1>(a, smask, 0u); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
-            release();
-            st = acquire();
-            k0.load(st);                                     // (1,3) (2,3)
-            k0.get<0>(a, smask, 0u); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
-            k0.get<1>(a, smask, 0u); mv(hp[2], a, mq); mvT(cq, a, mp[2]);
+            k1.get<1>(a); mv(hp[0], a, mq); mvT(cq, a, mp[0]);
+            k0.load(st + 2 * kSymvCoupleBytes);              // (1,3) (2,3)
+            k0.get<0>(a); mv(hp[1], a, mq); mvT(cq, a, mp[1]);
+            k0.get<1>(a); mv(hp[2], a, mq); mvT(cq, a, mp[2]);
 #pragma unroll
             for (int c = 0; c < 3; ++c) hp[3][c] = cadd(hp[3][c], shfl2(cq[c], src));
             // (r, r): rows 0, 1 in the lower strip's couple, rows 2, 3 in the upper strip's; each strip does its own
             // direction of the product (the upper one with the transpose)
-            k0.load(st + kSymvCoupleBytes + (lower ? 0u : other));
-            k1.load(st + kSymvCoupleBytes + (lower ? other : 0u));
+            k0.load(st + 3 * kSymvCoupleBytes + (lower ? 0u : other));
+            k1.load(st + 3 * kSymvCoupleBytes + (lower ? other : 0u));
 #pragma unroll
             for (int c = 0; c < 3; ++c) mq[c] = shfl2(mp[0][c], src);
-            k0.get<0>(a, smask, tmask); mv(hp[0], a, mq);
+            k0.get<0>(a, tmask); mv(hp[0], a, mq);
 #pragma unroll
             for (int c = 0; c < 3; ++c) mq[c] = shfl2(mp[1][c], src);
-            k0.get<1>(a, smask, tmask); mv(hp[1], a, mq);
+            k0.get<1>(a, tmask); mv(hp[1], a, mq);
 #pragma unroll
             for (int c = 0; c < 3; ++c) mq[c] = shfl2(mp[2][c], src);
-            k1.get<0>(a, smask, tmask); mv(hp[2], a, mq);
+            k1.get<0>(a, tmask); mv(hp[2], a, mq);
 #pragma unroll
             for (int c = 0; c < 3; ++c) mq[c] = shfl2(mp[3][c], src);
-            k1.get<1>(a, smask, tmask); mv(hp[3], a, mq);
+            k1.get<1>(a, tmask); mv(hp[3], a, mq);
             release();
         }
 
@@ -296,23 +310,21 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
             uint32_t st = acquire();
             k0.load(st);                                     // (0,0) (1,1)
             k1.load(st + kSymvCoupleBytes);                  // (2,2) (3,3)
-            k0.get<0>(a, smask, 0u); mv(hp[0], a, mp[0]);
-            k0.get<1>(a, smask, 0u); mv(hp[1], a, mp[1]);
-            k1.get<0>(a, smask, 0u); mv(hp[2], a, mp[2]);
-            k1.get<1>(a, smask, 0u); mv(hp[3], a, mp[3]);
-            release();
-            st = acquire();
-            k0.load(st);                                     // (0,1) (0,2)
-            k1.load(st + kSymvCoupleBytes);                  // (0,3) (1,2)
-            k0.get<0>(a, smask, 0u); mv(hp[0], a, mp[1]); mvT(hp[1], a, mp[0]);
-            k0.get<1>(a, smask, 0u); mv(hp[0], a, mp[2]); mvT(hp[2], a, mp[0]);
-            k1.get<0>(a, smask, 0u); mv(hp[0], a, mp[3]); mvT(hp[3], a, mp[0]);
-            k1.get<1>(a, smask, 0u); mv(hp[1], a, mp[2]); mvT(hp[2], a, mp[1]);
+            k0.get<0>(a); mv(hp[0], a, mp[0]);
+            k0.get<1>(a); mv(hp[1], a, mp[1]);
+            k1.get<0>(a); mv(hp[2], a, mp[2]);
+            k1.get<1>(a); mv(hp[3], a, mp[3]);
+            k0.load(st + 2 * kSymvCoupleBytes);              // (0,1) (0,2)
+            k1.load(st + 3 * kSymvCoupleBytes);              // (0,3) (1,2)
+            k0.get<0>(a); mv(hp[0], a, mp[1]); mvT(hp[1], a, mp[0]);
+            k0.get<1>(a); mv(hp[0], a, mp[2]); mvT(hp[2], a, mp[0]);
+            k1.get<0>(a); mv(hp[0], a, mp[3]); mvT(hp[3], a, mp[0]);
+            k1.get<1>(a); mv(hp[1], a, mp[2]); mvT(hp[2], a, mp[1]);
             release();
             st = acquire();
             k0.load(st);                                     // (1,3) (2,3)   (short stage: one couple)
-            k0.get<0>(a, smask, 0u); mv(hp[1], a, mp[3]); mvT(hp[3], a, mp[1]);
-            k0.get<1>(a, smask, 0u); mv(hp[2], a, mp[3]); mvT(hp[3], a, mp[2]);
+            k0.get<0>(a); mv(hp[1], a, mp[3]); mvT(hp[3], a, mp[1]);
+            k0.get<1>(a); mv(hp[2], a, mp[3]); mvT(hp[3], a, mp[2]);
             release();
         }
 
@@ -323,8 +335,8 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
             if (act && layer < nz) {
                 const float sc = __ldg(inv_dz + layer);
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
-                    sts(my_slot + (uint32_t)(c * nz + layer) * row_bytes, cscale(sc, hp[r][c]));
+                for (int c = 0; c < 3; ++c)                  // c == 1 on the mirror slot: back from D H^
+                    sts(my_slot + (uint32_t)(c * nz + layer) * row_bytes, cscale(c == 1 ? fxor(sc, smask) : sc, hp[r][c]));
             }
         }
         __syncthreads();
@@ -349,11 +361,11 @@ size_t coupling_symv_bank_bytes(int nz, long long n_tiles) {
 }
 
 cudaError_t launch_coupling_symv(const CouplingArgs& a, cudaStream_t st) {
-    constexpr int NWARP = kSymvWarps, NS = 4, MINB = 2;
+    constexpr int NWARP = kSymvWarps, NS = 2, MINB = 2;       // ring: two stages of four couples per warp
     const SymvGeom G = symv_geom(a.nz);
     if (a.tile_k != 2 * NWARP * G.EPW) return cudaErrorInvalidValue;
     auto kern = coupling_symv_kernel<NWARP, NS, MINB>;
-    const size_t smem = ((NWARP * NS * 8 + 127) & ~127) + (size_t)NWARP * NS * kSymvStageBytes +
+    const size_t smem = ((NWARP * NS * 8 + 127) & ~127) + (size_t)NWARP * NS * 4 * kSymvCoupleBytes +
                         (size_t)3 * a.nz * NWARP * G.EPW * 16;
     static PerDevice<int> cache;
     int occ = 1;
