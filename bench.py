@@ -320,10 +320,12 @@ def sweep_nz():
         m /= m.norm(dim=1, keepdim=True)
         h = torch.empty_like(m)
         dz_var = np.exp(np.random.default_rng(SEED_SWEEP + nz).uniform(np.log(0.3), np.log(3.0), size=nz))
-        for name, dz, kw in [("hybrid (ky-mirror bank)", dz_var, dict(dedup=0)),
-                             ("hybrid (plain bank)", dz_var, dict(dedup=0, mirror=0)),
-                             ("equidistant, Toeplitz classes", np.full(nz, 1.0), dict(dedup=2)),
-                             ("equidistant, z-FFT (Eq.25)", np.full(nz, 1.0), dict(dedup=3))]:
+        for name, dz, kw in [("hybrid, automatic (reciprocity / ky-mirror bank)", dz_var, dict()),
+                             ("hybrid, ky-mirror bank (recip 0)", dz_var, dict(dedup=0, recip=0)),
+                             ("hybrid, plain bank (mirror 0)", dz_var, dict(dedup=0, mirror=0)),
+                             ("equidistant, automatic", np.full(nz, 1.0), dict()),
+                             ("equidistant, Toeplitz classes (dedup 2)", np.full(nz, 1.0), dict(dedup=2)),
+                             ("equidistant, z-FFT of Eq.25 (dedup 3)", np.full(nz, 1.0), dict(dedup=3))]:
             if kw.get("mirror") == 0 and nz > 64:
                 continue                                     # plain bank of 29 / 52 GB: not needed for the comparison
             plan = hb.Plan(nx, ny, nz, 2.0, 2.0, dz, "f32", **kw)

@@ -182,30 +182,42 @@ static cudaError_t upload_inv_dz(hfft_plan* p) {
 static void plan_sizes(hfft_plan* p) {
     const size_t e = p->elem;
     p->n_k = 2LL * p->ny * (p->nx + 1);
-    // deduplicated bank: automatically once at most half of the pairs carry a tensor of their own
-    p->dedup = p->dedup_mode == 2 || (p->dedup_mode == 1 && 2 * p->n_classes <= p->nz * p->nz);
-    // equal thicknesses: the z-convolution by FFT (PAPER.md:182 Eq.25) where it applies, from 16 layers on
-    // (below that the explicit Toeplitz sum does less work)
-    p->zfft = p->toeplitz && coupling_zfft_applies(p->nz, e, &p->log2lz) &&
-              (p->dedup_mode == 3 || (p->dedup_mode == 1 && p->nz >= 16));
-    if (p->zfft) p->dedup = true;
-    p->class_kernel = p->dedup && !p->zfft &&
-                      coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
-    // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
     const int wide = 32 * (int)(16 / e);
     const bool big = p->n_k / wide >= 2LL * (p->num_sms > 0 ? p->num_sms : 148);
-    p->tile_k = big ? wide : 32;
-    while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
-    if (p->tile_k != wide) p->tile_k = 32;
-    if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
-    if (p->class_kernel || p->zfft) p->tile_k = 32;
     // ky-mirror storage (the spectra are even or odd in ky): where the plain streaming kernel would run
     // with wide tiles (mode 2: on any grid) it reads one bank value per pair (ky, 2ny - ky); the spectrum rows then
     // have 2ny + 2 slots (fft_kernels.cu ypos).  Tiles of 64 slots = 32 bank entries, one per lane, in both
     // precisions: measured faster than 128-slot tiles in fp32 (B200, C4: 1.11 vs 1.28 ms, C3: 0.084 vs 0.098 ms --
     // two or more CTAs with their M^ tiles share an SM).
-    p->mirror = p->mirror_mode >= 1 && !p->dedup && (big || p->mirror_mode == 2) && p->ny >= 2 &&
-                !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
+    const bool mirror_ok = p->mirror_mode >= 1 && (big || p->mirror_mode == 2) && p->ny >= 2 &&
+                           !coupling_batched_applies(p->nz, p->batch, e) && coupling_smem_bytes(p->nz, 64, e) <= 200 * 1024;
+    // equal thicknesses: the z-convolution by FFT (PAPER.md:182 Eq.25) where it applies, from 16 layers on
+    // (below that the explicit Toeplitz sum does less work)
+    p->zfft = p->toeplitz && coupling_zfft_applies(p->nz, e, &p->log2lz) &&
+              (p->dedup_mode == 3 || (p->dedup_mode == 1 && p->nz >= 16));
+    // deduplicated bank (mode 2: always).  Automatic mode: once at most half of the pairs carry a tensor of their own
+    // AND the class path is the faster one.  Measured on B200 at 256 x 256 fp32 (profiles/r02_scaling_nz.md): the z-FFT
+    // and the Toeplitz window kernel always win; the generic class kernel (bank tile in shared memory, bound by its
+    // bandwidth) wins up to 8 layers and loses to the mirror / reciprocity bank from 16 on (nz = 32: 0.35 vs 0.28 ms),
+    // the class-indexed streaming fallback (tile too large for shared memory) loses by 1.5-2x (nz = 64: 1.53 vs 0.79 ms)
+    // -- so those two are chosen only where the mirror storage does not apply (small grids, nz > 133 in fp32).
+    const bool few = 2 * p->n_classes <= p->nz * p->nz;
+    const bool fits = coupling_class_smem_bytes(p->nz, p->n_classes, p->toeplitz, e) <= 220 * 1024;
+    bool auto_dedup = few;
+    if (few && mirror_ok && !p->zfft) {
+        if (!fits) auto_dedup = false;                               // streaming fallback
+        else if (!p->toeplitz && p->nz > 8) auto_dedup = false;      // generic class kernel
+    }
+    p->dedup = p->dedup_mode == 2 || (p->dedup_mode == 1 && auto_dedup);
+    if (p->zfft) p->dedup = true;
+    p->class_kernel = p->dedup && !p->zfft && fits;
+    // wide tiles (128-bit bank loads per lane) once there are enough of them to fill the chip twice
+    p->tile_k = big ? wide : 32;
+    while (p->tile_k > 32 && coupling_smem_bytes(p->nz, p->tile_k, e) > 200 * 1024) p->tile_k /= 2;
+    if (p->tile_k != wide) p->tile_k = 32;
+    if (!p->dedup && coupling_batched_applies(p->nz, p->batch, e)) p->tile_k = 32;
+    if (p->class_kernel || p->zfft) p->tile_k = 32;
+    p->mirror = mirror_ok && !p->dedup;
     if (p->mirror) p->tile_k = 64;
     // reciprocity storage on top of the mirror storage.  fp32, nz <= 64: the symv layout, every block read
     // once and used for both of its layer pairs (coupling_symv.cu) -- automatic from 8 layers on where it streams at
