@@ -212,6 +212,186 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
     cp_async_wait_group<0>();
 }
 
+// ---- long stacks (Lz = 128, 256; fp32): the same transform with the spectra kept in SHARED memory between the steps ----
+// coupling_zfft_kernel holds all three components of a thread's layers in registers (3 x 16 complex = 96 registers at
+// Lz >= 128): one 8-warp CTA per SM at Lz = 128 (ncu: 12 % warps active, latency bound at 4.2 TB/s) and spills at
+// Lz = 256.  Here a thread never holds more than one 16-point transform (or three 8-point ones): the forward and the
+// inverse first-stage transforms go component by component, the second-stage transform, the multiply by S(k, kz) and the
+// inverse second stage work in place in the exchange buffer on the thread's own (r, all s) entries -- no extra barrier.
+// Lz = 128: three 8-point transforms at a time, two CTAs per SM (measured slower than the register form, kept for A/B);
+// Lz = 256 (the shipped use): 16-point transforms component by component, then the multiply four kz at a time, 16 warps
+// per CTA.  The S values are read straight from global memory
+// (streaming loads, 128 B per warp and value), issued ahead of the shared-memory work that hides them.
+template <int LOG2LZ> struct Z2Cfg {
+    static constexpr int TT = ZCfg<LOG2LZ>::TT;
+    static constexpr int THREADS = 32 * TT;
+    static constexpr int MINB = TT <= 8 ? 2 : 1;
+    static constexpr size_t SMEM = (size_t)3 * ZCfg<LOG2LZ>::LZ * 32 * sizeof(float2) + ZCfg<LOG2LZ>::LZ * sizeof(float2);
+};
+
+template <int LOG2LZ>
+__global__ void __launch_bounds__(Z2Cfg<LOG2LZ>::THREADS, Z2Cfg<LOG2LZ>::MINB)
+coupling_zfft2_kernel(const float* __restrict__ bank3, float2* __restrict__ spec, const float2* __restrict__ twz, int nz,
+                      int batch, long long n_tiles, long long ks) {
+    typedef float T;
+    typedef float2 C;
+    typedef ZCfg<LOG2LZ> Z;
+    constexpr int LZ = Z::LZ, E = Z::E, TT = Z::TT, RPT = Z::RPT, TK = 32;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    C* ex = reinterpret_cast<C*>(smem_raw);                                   // [3][LZ][32]
+    C* stw = reinterpret_cast<C*>(smem_raw + (size_t)3 * LZ * TK * sizeof(C));  // [LZ] exp(-2 pi i n / LZ)
+    const int lane = threadIdx.x & 31, t = threadIdx.x >> 5;
+    const int np = 3 * nz;
+    for (int x = threadIdx.x; x < LZ; x += blockDim.x) stw[x] = twz[x];
+    const long long n_items = n_tiles * batch;
+    pdl_wait();                                             // M^ comes from the previous kernel (S2)
+    __syncthreads();
+
+    for (long long item = blockIdx.x; item < n_items; item += gridDim.x) {
+        const long long tile = item / batch;
+        const int b = (int)(item - tile * batch);
+        C* sp = spec + (long long)b * np * ks + tile * TK + lane;
+        const T* bt = bank3 + tile * LZ * (6LL * TK) + lane;
+        // ---- forward, first stage: DFT_E over q (upper half zero), twiddle W_LZ^{t r}; all loads first ----
+        {
+            C in[3][E / 2];
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int q = 0; q < E / 2; ++q) {
+                    const int n = t + TT * q;
+                    in[c][q] = n < nz ? sp[(long long)(c * nz + n) * ks] : mk<T>((T)0, (T)0);
+                }
+#pragma unroll
+            for (int c = 0; c < 3; ++c) {
+                C v[E];
+#pragma unroll
+                for (int q = 0; q < E / 2; ++q) v[q] = in[c][q];
+                rdft<E, false, true, T>(v);
+#pragma unroll
+                for (int r = 1; r < E; ++r) v[r] = cmul(v[r], stw[(t * r) & (LZ - 1)]);
+#pragma unroll
+                for (int r = 0; r < E; ++r) ex[((c * LZ) + r * TT + t) * TK + lane] = v[r];
+            }
+        }
+        __syncthreads();
+        // ---- second stage, multiply, inverse second stage: in place on this thread's entries (r = t RPT + rr, all s) ----
+        if constexpr (TT <= 8) {
+#pragma unroll 1
+            for (int rr = 0; rr < RPT; ++rr) {
+                const int r = t * RPT + rr;
+                constexpr int HS = TT / 2;                   // S values in two batches: 24 registers at a time
+                T a[HS][6];
+#pragma unroll
+                for (int s = 0; s < HS; ++s)
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * s) * 6 + c) * TK);
+                C w[3][TT];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+#pragma unroll
+                    for (int s = 0; s < TT; ++s) w[c][s] = ex[((c * LZ) + r * TT + s) * TK + lane];
+                    rdft<TT, false, false, T>(w[c]);
+                }
+#pragma unroll
+                for (int half = 0; half < 2; ++half) {
+#pragma unroll
+                    for (int s = 0; s < HS; ++s) {           // kz = r + E (half HS + s)
+                        const int o = half * HS + s;
+                        const C mx = w[0][o], my = w[1][o], mz = w[2][o];
+                        C hx = cscale(a[s][0], mx), hy = cscale(a[s][3], mx), hz = cscale(a[s][4], mx);
+                        hx = caxpy(a[s][3], my, hx); hy = caxpy(a[s][1], my, hy); hz = caxpy(a[s][5], my, hz);
+                        hx = caxpy(a[s][4], mz, hx); hy = caxpy(a[s][5], mz, hy); hz = caxpy(a[s][2], mz, hz);
+                        w[0][o] = hx; w[1][o] = hy; w[2][o] = hz;
+                    }
+                    if (half == 0) {
+#pragma unroll
+                        for (int s = 0; s < HS; ++s)
+#pragma unroll
+                            for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * (HS + s)) * 6 + c) * TK);
+                    }
+                }
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    rdft<TT, true, false, T>(w[c]);
+#pragma unroll
+                    for (int s = 0; s < TT; ++s) ex[((c * LZ) + r * TT + s) * TK + lane] = w[c][s];
+                }
+            }
+        } else {
+            static_assert(RPT == 1 || TT <= 8, "one r per thread in the component-by-component form");
+            const int r = t;
+#pragma unroll 1
+            for (int c = 0; c < 3; ++c) {
+                C w[TT];
+#pragma unroll
+                for (int s = 0; s < TT; ++s) w[s] = ex[((c * LZ) + r * TT + s) * TK + lane];
+                rdft<TT, false, false, T>(w);
+#pragma unroll
+                for (int s = 0; s < TT; ++s) ex[((c * LZ) + r * TT + s) * TK + lane] = w[s];
+            }
+#pragma unroll 1
+            for (int s0 = 0; s0 < TT; s0 += 4) {
+                T a[4][6];
+#pragma unroll
+                for (int s = 0; s < 4; ++s)
+#pragma unroll
+                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * (s0 + s)) * 6 + c) * TK);
+#pragma unroll
+                for (int s = 0; s < 4; ++s) {
+                    C* e0 = ex + (r * TT + s0 + s) * TK + lane;
+                    const C mx = e0[0], my = e0[LZ * TK], mz = e0[2 * LZ * TK];
+                    C hx = cscale(a[s][0], mx), hy = cscale(a[s][3], mx), hz = cscale(a[s][4], mx);
+                    hx = caxpy(a[s][3], my, hx); hy = caxpy(a[s][1], my, hy); hz = caxpy(a[s][5], my, hz);
+                    hx = caxpy(a[s][4], mz, hx); hy = caxpy(a[s][5], mz, hy); hz = caxpy(a[s][2], mz, hz);
+                    e0[0] = hx; e0[LZ * TK] = hy; e0[2 * LZ * TK] = hz;
+                }
+            }
+#pragma unroll 1
+            for (int c = 0; c < 3; ++c) {
+                C w[TT];
+#pragma unroll
+                for (int s = 0; s < TT; ++s) w[s] = ex[((c * LZ) + r * TT + s) * TK + lane];
+                rdft<TT, true, false, T>(w);
+#pragma unroll
+                for (int s = 0; s < TT; ++s) ex[((c * LZ) + r * TT + s) * TK + lane] = w[s];
+            }
+        }
+        __syncthreads();
+        // ---- inverse first stage, component by component; crop to the layers n < nz <= LZ / 2 ----
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            C v[E];
+#pragma unroll
+            for (int r = 0; r < E; ++r) v[r] = ex[((c * LZ) + r * TT + t) * TK + lane];
+#pragma unroll
+            for (int r = 1; r < E; ++r) v[r] = cmulc(v[r], stw[(t * r) & (LZ - 1)]);
+            rdft<E, true, false, T>(v);
+#pragma unroll
+            for (int q = 0; q < E / 2; ++q) {
+                const int n = t + TT * q;
+                if (n < nz) sp[(long long)(c * nz + n) * ks] = v[q];
+            }
+        }
+        __syncthreads();                                     // the exchange buffer is free again
+    }
+}
+
+template <int L>
+static cudaError_t launch_zfft2_l(const CouplingArgs& a, cudaStream_t st) {
+    auto kern = coupling_zfft2_kernel<L>;
+    const size_t smem = Z2Cfg<L>::SMEM;
+    static PerDevice<int> cache;
+    int occ = 1;
+    cudaError_t err = ctas_per_sm_cached(kern, Z2Cfg<L>::THREADS, smem, cache, occ);
+    if (err != cudaSuccess) return err;
+    const long long items = a.n_tiles * a.batch;
+    long long grid = (long long)a.num_sms * occ;
+    if (grid > items) grid = items;
+    return launch_pdl(kern, dim3((unsigned)grid), dim3(Z2Cfg<L>::THREADS), smem, st, (const float*)a.bank, (float2*)a.spec,
+                      (const float2*)a.twz, a.nz, a.batch, a.n_tiles, a.ks);
+}
+
 // ---- setup: z-DFT of the Toeplitz classes ----
 // cls64: [nz][6][kstride] fp64 (class d = i - j >= 0, plain layout); twz64: exp(-2 pi i n / LZ)
 template <typename T>
@@ -289,8 +469,13 @@ cudaError_t launch_coupling_zfft(const CouplingArgs& a, cudaStream_t st) {
         default: break;
     }
     if constexpr (sizeof(T) == 4) {
-        if (a.log2lz == 7) return launch_zfft_l<T, 7>(a, st);
-        if (a.log2lz == 8) return launch_zfft_l<T, 8>(a, st);
+        // Lz = 128: the register-resident kernel (B200, 256 x 256 x 64: S3 0.193 ms against 0.357 ms for the shared-memory
+        // form, which pays two more trips through the exchange buffer); Lz = 256: the shared-memory form (no spills:
+        // evaluation 1.13 -> 0.81 ms at nz = 128, 1.02 -> 0.69 ms at nz = 96).  HFFT_ZFFT_FORM=reg|smem forces one (A/B).
+        static const char* form = getenv("HFFT_ZFFT_FORM");
+        const bool smem_form = form ? form[0] == 's' : a.log2lz == 8;
+        if (a.log2lz == 7) return smem_form ? launch_zfft2_l<7>(a, st) : launch_zfft_l<T, 7>(a, st);
+        if (a.log2lz == 8) return smem_form ? launch_zfft2_l<8>(a, st) : launch_zfft_l<T, 8>(a, st);
     }
     return cudaErrorInvalidValue;
 }
