@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--mirror", type=int, default=None, help="hfft_plan_set_mirror mode (default: the library's, 1)")
     ap.add_argument("--recip", type=int, default=None, help="hfft_plan_set_recip (default: the library's)")
     ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
+    ap.add_argument("--fusion", type=int, default=None, help="hfft_plan_set_fusion mode (default: the library's, 1)")
     ap.add_argument("--all-configs", action="store_true",
                     help="run every config (1, 2, 2f64, 3, 4, 4eq, 5) in a process of its own and write the bench lines, "
                          "with their clocks, as a markdown table + JSON lines to --out")
@@ -73,7 +74,7 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md)"
 
 
-def algorithmic_bytes(w, n_slots=None, mirror=False, recip=False):
+def algorithmic_bytes(w, n_slots=None, mirror=False, recip=False, fused=False):
     """what the method must move per hfft_demag call with the symmetries the storage
     uses.  n_slots: bank slots per wavevector (nz^2 pairs, or the tensor classes of a deduplicated bank);
     mirror: ky-mirror storage, one bank entry per (kx, ky <= ny); recip: reciprocity, one block per unordered
@@ -89,6 +90,9 @@ def algorithmic_bytes(w, n_slots=None, mirror=False, recip=False):
     field = planes * w.ny * w.nx * s
     coupling = bank + 2 * spec
     whole = 2 * field + 4 * xhat + 4 * spec + bank
+    if fused:                              # S2 + S3 + S4 in one kernel: X^ in, X^ out, the spectra stay in shared memory
+        coupling = bank + 2 * xhat
+        whole = 2 * field + 4 * xhat + bank
     return {"bank": bank, "coupling": coupling, "whole": whole}
 
 
@@ -388,7 +392,7 @@ def all_configs(args):
                  "| whole / roofline | bank | SM MHz (median / max) | throttle reasons |\n|---|---:|---:|---:|---|---|---:|---|---|---|\n")
         for d in lines:
             r, st, ck, bk = d["roofline"], d["stages_ms"], d["clocks"], d["bank"]
-            kind = ("z-FFT" if bk["dedup"] == 4 else "classes" if bk["dedup"] else "symv" if bk["symv_layout"] else
+            kind = ("fused S2+S3+S4, plain" if bk.get("fused_s2s3s4") else "z-FFT" if bk["dedup"] == 4 else "classes" if bk["dedup"] else "symv" if bk["symv_layout"] else
                     "recip" if bk["reciprocity"] else "mirror" if bk["ky_mirror"] else "plain")
             fh.write("| %s | %.4f | %.1f | %.1f | %s | %s %.4g / %.4g %s = %.2f | %.2f | %s, %.3f GB | %s / %s | %s |\n" % (
                 d["config"]["workload"], d["ms_per_step"], d["value"], d["e2e"]["value"],
@@ -432,7 +436,7 @@ def main():
         torch.cuda.synchronize()
 
     plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, batch=w.B, dedup=args.dedup, mirror=args.mirror,
-                   recip=args.recip)
+                   recip=args.recip, fusion=args.fusion)
     t0 = time.perf_counter()
     plan.build_tensor()
     torch.cuda.synchronize()
@@ -451,7 +455,8 @@ def main():
     recip = int(plan.info.mirror) >= 2                     # 2: p <= q storage read twice, 3: symv layout read once
     symv = int(plan.info.mirror) == 3
     slots = int(plan.info.bank_bytes // (6 * (plan.info.n_k_padded // (2 if mirror else 1)) * (4 if w.precision == "f32" else 8)))
-    ab = algorithmic_bytes(w, slots if dedup else None, mirror, recip)
+    fused = bool(plan.info.fused)
+    ab = algorithmic_bytes(w, slots if dedup else None, mirror, recip, fused)
     # inputs larger than L2?  otherwise flush L2 between steps (l2_mode: the same rule, printed in `config`)
     flush = None
     if l2_mode(w).startswith("L2 flushed") or ab["whole"] < (256 << 20):
@@ -606,6 +611,9 @@ def main():
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},
             "setup_s": setup_s,
         }
+        if fused:
+            line["roofline"]["kernel"] = ("fused_ycy_kernel (S2 + S3 + S4 in one launch: y transforms and coupling of one kx "
+                                          "column of all planes, spectra in shared memory; stages_ms charges it to `coupling`)")
         if ms_graph is not None:
             line["cuda_graph"] = {"ms_per_step": ms_graph, "evals_per_s": w.B / (ms_graph * 1e-3),
                                   "note": "the same hfft_demag captured once and replayed (timed like the main region)"}
@@ -624,7 +632,7 @@ def main():
                                 "unit": "TFLOP/s", "frac": tf / alu_peak if tf else None,
                                 "algorithmic_flops_per_launch": flops, "avg_launch_ms": coup_ms,
                                 "hbm_gbs": achieved, "traffic": None}
-        line["bank"] = {"dedup": dedup, "ky_mirror": mirror, "reciprocity": recip, "symv_layout": symv,
+        line["bank"] = {"dedup": dedup, "ky_mirror": mirror, "reciprocity": recip, "symv_layout": symv, "fused_s2s3s4": fused,
                         "slots_per_k": slots, "bytes": int(plan.info.bank_bytes)}
         line["l2_flush_between_steps"] = flush is not None
         if world == 1 and not args.no_cpu_baseline:

@@ -79,7 +79,7 @@ typedef struct {
     size_t workspace_bytes;   /* spectra X^, M^ (H^ overwrites M^).  The host paths allocate their staging copies of
                                  m and h themselves, on first use */
     size_t setup_scratch_bytes; /* allocated inside hfft_build_tensor and freed before it returns */
-    int launches_per_demag;   /* kernels hfft_demag enqueues per call */
+    int launches_per_demag;   /* kernels hfft_demag enqueues per call: 5, or 3 with the fused S2+S3+S4 kernel */
     int built;                /* 1 once hfft_build_tensor has completed */
     int n_classes;            /* bank slots a deduplicated bank needs: distinct tensors among the nz^2 layer pairs;
                                  nz for equal thicknesses (N_ij and N_ji then differ by the sign of xz, yz only) */
@@ -90,6 +90,7 @@ typedef struct {
     int dedup;                /* 0: one bank slot per pair; 1: per class, streamed; 2: per class, bank tile in
                                  shared memory; 3: as 2 with Toeplitz classes (equal thicknesses); 4: equal
                                  thicknesses, z-convolution by FFT (Eq.25) */
+    int fused;                /* 1: S2 + S3 + S4 run as one kernel (hfft_plan_set_fusion) */
 } hfft_info;
 
 /*
@@ -171,6 +172,21 @@ hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
  * hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
+
+/* Fusion of the layer coupling into the y transforms (north_star (c); the F2^-1 [ sum_j3 ... ] F2 sandwich of Eq.24,
+ * PAPER.md:177-178): stages S2, S3 and S4 run as ONE kernel in which a CTA takes the kx column of all 3 nz planes --
+ * forward y transforms, coupling in shared memory, inverse y transforms -- so that M^ / H^ never reach global memory
+ * and hfft_demag enqueues 3 kernels instead of 5 (info.fused == 1, info.launches_per_demag == 3).  It needs the plain
+ * bank (no ky-mirror, reciprocity or deduplicated storage), the column 3 nz x 2ny complex plus the transform rows
+ * within 222 KB of shared memory, nz <= 32, and no batched coupling.
+ *   mode = 1 (default): automatic -- on the small grids (those too small for the wide-tile / mirror storage), which
+ *          are bound by kernel launches; large grids keep the staged path with its smaller banks, which is faster
+ *          there (measured: profiles/r02_fusion.md).
+ *   mode = 2: wherever it fits (overrides the automatic ky-mirror / reciprocity storage, not hfft_plan_set_mirror(2)).
+ *   mode = 0: never.
+ * Must be called before hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
+ */
+hfft_status hfft_plan_set_fusion(hfft_plan *plan, int mode);
 
 /*
  * Host-only helper (no device needed): the tensor classes hfft_plan_set_dedup works with.

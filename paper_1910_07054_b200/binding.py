@@ -23,7 +23,7 @@ STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
 
 # every symbol include/hfft.h declares
-EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror", "hfft_plan_set_recip",
+EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror", "hfft_plan_set_recip", "hfft_plan_set_fusion",
            "hfft_tensor_classes", "hfft_plan_info", "hfft_bank_bytes", "hfft_workspace_bytes", "hfft_plan_set_buffers",
            "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
@@ -37,7 +37,7 @@ class Info(ctypes.Structure):
                 ("bank_bytes", ctypes.c_size_t), ("workspace_bytes", ctypes.c_size_t),
                 ("setup_scratch_bytes", ctypes.c_size_t),
                 ("launches_per_demag", ctypes.c_int), ("built", ctypes.c_int),
-                ("n_classes", ctypes.c_int), ("mirror", ctypes.c_int), ("dedup", ctypes.c_int)]
+                ("n_classes", ctypes.c_int), ("mirror", ctypes.c_int), ("dedup", ctypes.c_int), ("fused", ctypes.c_int)]
 
 
 class HfftError(RuntimeError):
@@ -65,6 +65,7 @@ def lib():
         L.hfft_plan_set_dedup.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_mirror.argtypes = [vp, ctypes.c_int]
         L.hfft_plan_set_recip.argtypes = [vp, ctypes.c_int]
+        L.hfft_plan_set_fusion.argtypes = [vp, ctypes.c_int]
         L.hfft_tensor_classes.argtypes = [ctypes.c_int, dp, ip, ip, ip]
         L.hfft_plan_info.argtypes = [vp, ctypes.POINTER(Info)]
         L.hfft_bank_bytes.argtypes = [vp]
@@ -139,6 +140,11 @@ def workspace_bytes(plan) -> int:
 
 def plan_set_mirror(plan, on):
     _check(lib().hfft_plan_set_mirror(plan, int(on)), plan)
+
+
+def plan_set_fusion(plan, mode):
+    """0 off, 1 automatic (default: small grids), 2 wherever the fused S2+S3+S4 kernel fits."""
+    _check(lib().hfft_plan_set_fusion(plan, int(mode)), plan)
 
 
 def plan_set_recip(plan, on):
@@ -241,7 +247,7 @@ def destroy(plan):
 class Plan:
     """Convenience owner: plan + torch-allocated bank / workspace on the current CUDA device."""
 
-    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None, mirror=None, recip=None):
+    def __init__(self, nx, ny, nz, dx, dy, dz, precision="f32", batch=1, torch_buffers=True, dedup=None, mirror=None, recip=None, fusion=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -259,6 +265,8 @@ class Plan:
             plan_set_mirror(self.handle, mirror)
         if recip is not None:
             plan_set_recip(self.handle, recip)
+        if fusion is not None:
+            plan_set_fusion(self.handle, fusion)
         self.info = plan_info(self.handle)
         self._bank = self._ws = None
         if torch_buffers:

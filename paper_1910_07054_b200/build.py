@@ -16,7 +16,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libhfft.so")
-SOURCES = ["hfft_api.cu", "fft_kernels.cu", "coupling.cu", "coupling_symv.cu", "coupling_zfft.cu", "tensor_build.cu"]
+SOURCES = ["hfft_api.cu", "fft_kernels.cu", "coupling.cu", "coupling_symv.cu", "coupling_zfft.cu", "fused_ycy.cu", "tensor_build.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 COMMON = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 # error-free transforms of the double-double setup code must not be re-associated or contracted

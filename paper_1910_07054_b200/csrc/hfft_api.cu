@@ -51,6 +51,8 @@ struct hfft_plan {
     bool symv = false;                               // ... in the symv layout, read once by coupling_symv_kernel
     std::vector<int> recip_cls, recip_rep;           // pair -> slot of the unordered pair; slot -> p*nz+q (p <= q)
     void* d_invdz = nullptr;                         // 1 / dz_i, plan precision (recip)
+    int fuse_mode = 1;                               // hfft_plan_set_fusion: 0 off, 1 automatic (small grids), 2 wherever it fits
+    bool fused = false;                              // S2 + S3 + S4 in one kernel (fused_ycy.cu)
     int mirror_mode = 1;                             // hfft_plan_set_mirror: 0 off, 1 automatic
     bool mirror = false;                             // spectrum in the mirror layout, half bank (coupling_kernel MIR)
     long long n_slots = 0;                           // spectrum slots per plane before padding
@@ -219,6 +221,16 @@ static void plan_sizes(hfft_plan* p) {
     if (p->class_kernel || p->zfft) p->tile_k = 32;
     p->mirror = mirror_ok && !p->dedup;
     if (p->mirror) p->tile_k = 64;
+    // S2 + S3 + S4 fused (fused_ycy.cu): plain bank in 32-wavevector tiles, the kx column of all planes in one CTA's
+    // shared memory.  Automatic on the small grids only (those that do not fill the chip with wide tiles: they are bound
+    // by launches, not bytes -- B200, 64 x 64 x 6: 22.8 -> see DESIGN.md 8); mode 2 forces it wherever it fits.
+    {
+        const size_t fs = fused_ycy_smem_bytes(p->log2ny + 1, p->nz, e);
+        p->fused = p->fuse_mode >= 1 && !p->dedup && !p->zfft &&
+                   (p->fuse_mode == 2 || !coupling_batched_applies(p->nz, p->batch, e)) && fs > 0 && fs <= 222 * 1024 &&
+                   (p->fuse_mode == 2 ? p->mirror_mode != 2 : !p->mirror && !big && fused_ycy_pays(p->log2ny + 1, p->nz, e));
+        if (p->fused) { p->mirror = false; p->tile_k = 32; }
+    }
     // reciprocity storage on top of the mirror storage.  fp32, nz <= 64: the symv layout, every block read
     // once and used for both of its layer pairs (coupling_symv.cu) -- automatic from 8 layers on where it streams at
     // least 30 % fewer bytes than the mirror bank (the layout pads nz to whole strips of 4, the strips to a power of two);
@@ -342,6 +354,15 @@ hfft_status hfft_plan_set_mirror(hfft_plan* plan, int on) {
     return HFFT_OK;
 }
 
+hfft_status hfft_plan_set_fusion(hfft_plan* plan, int mode) {
+    if (!plan) return HFFT_EINVAL;
+    if (mode < 0 || mode > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_fusion: 0, 1 or 2");
+    if (plan->built || plan->ws) return fail(plan, HFFT_ESTATE, "hfft_plan_set_fusion: after build / set_buffers");
+    plan->fuse_mode = mode;
+    plan_sizes(plan);
+    return HFFT_OK;
+}
+
 hfft_status hfft_plan_set_recip(hfft_plan* plan, int on) {
     if (!plan) return HFFT_EINVAL;
     if (on < 0 || on > 2) return fail(plan, HFFT_EINVAL, "hfft_plan_set_recip: 0, 1 or 2");
@@ -372,7 +393,8 @@ hfft_status hfft_plan_info(const hfft_plan* plan, hfft_info* info) {
     info->bank_bytes = plan->bank_bytes; info->workspace_bytes = plan->ws_bytes;
     BuildGeom g = make_geom(plan);
     info->setup_scratch_bytes = build_scratch_bytes(g);
-    info->launches_per_demag = HFFT_NUM_STAGES;
+    info->launches_per_demag = plan->fused ? 3 : HFFT_NUM_STAGES;
+    info->fused = plan->fused ? 1 : 0;
     info->built = plan->built ? 1 : 0;
     info->n_classes = plan->n_classes;
     info->mirror = plan->mirror ? (plan->symv ? 3 : (plan->recip ? 2 : 1)) : 0;
@@ -490,6 +512,14 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
                                        p->num_sms, st)))
     // the z components are rotated by i on the k side (real form R6) except in the z-FFT mode
     const int nz_rot = p->zfft ? 0 : p->nz;
+    if (p->fused) {
+        // S2 + S3 + S4 in one launch; the profile charges it to the coupling stage (the two y stages read 0)
+        if (ev && ((e = cudaEventRecord(ev[1], st)) != cudaSuccess || (e = cudaEventRecord(ev[2], st)) != cudaSuccess))
+            return fail_cuda(p, "cudaEventRecord", e);
+        if ((e = launch_fused_ycy<T>(xhat, p->bank, p->nx, p->log2ny + 1, p->nz, p->batch, p->twt_y, p->num_sms, st)) != cudaSuccess)
+            return fail_cuda(p, "launch_fused_ycy", e);
+        if (ev && (e = cudaEventRecord(ev[3], st)) != cudaSuccess) return fail_cuda(p, "cudaEventRecord", e);
+    } else {
     STAGE(1, (launch_ffty_fwd<T, true>(xhat, spec, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y,
                                        p->num_sms, st, p->mirror ? 1 : 0)))
     CouplingArgs ca{p->bank, spec, p->nz, p->batch, p->tile_k, p->n_tiles, p->n_k_padded,
@@ -500,6 +530,7 @@ static hfft_status demag_impl(hfft_plan* p, const void* m, const double* Ms, voi
     STAGE(2, (launch_coupling<T>(ca, st)))
     STAGE(3, (launch_iffty<T>(spec, xhat, p->nx, p->log2ny + 1, planes, nz_rot, p->n_k_padded, p->twt_y, p->num_sms, st,
                               p->mirror ? 1 : 0)))
+    }
     if (p->sums && (e = cudaMemsetAsync(p->sums, 0, (size_t)planes * 2 * sizeof(double), st)) != cudaSuccess)
         return fail_cuda(p, "cudaMemsetAsync(sums)", e);
     STAGE(4, (launch_ifftx<T>(xhat, (T*)h, p->log2nx, planes, p->ny, p->tw_x, p->twt_x, p->num_sms, (const T*)m,

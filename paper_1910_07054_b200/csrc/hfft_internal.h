@@ -102,6 +102,13 @@ template <typename T>
 cudaError_t launch_iffty(const void* spec, void* xhat, int nx, int log2N, int nplanes, int nz_rot, long long ks,
                          const void* twt_N, int num_sms, cudaStream_t st, int mirror = 0);
 
+// ---- fused_ycy.cu: S2 + S3 + S4 in one kernel, one kx column of all planes per CTA (plain bank, tile_k == 32) ----
+size_t fused_ycy_smem_bytes(int log2N, int nz, size_t elem);   // 0: shape not supported
+bool fused_ycy_pays(int log2N, int nz, size_t elem);           // automatic mode: the bank slice fits shared memory too
+template <typename T>
+cudaError_t launch_fused_ycy(void* xhat, const void* bank, int nx, int log2N, int nz, int batch, const void* twt_N, int num_sms,
+                             cudaStream_t st);
+
 // ---- coupling.cu ----
 // H^ = bank * M^ in place on the k side.  bank layout [tile][class][6][tile_k]; class = i*nz+j (cls == nullptr)
 // or cls[i*nz+j] (deduplicated bank, device table).
