@@ -266,3 +266,29 @@ def test_repeated_calls_are_bitwise_identical(hb, case):
     for _ in range(25):
         assert torch.equal(plan.demag(m, w.Ms), first)
     plan.close()
+
+
+def test_automatic_mode_takes_a_class_path_only_where_it_was_measured_faster(hb):
+    """hfft_api.cu plan_sizes (numbers in profiles/r02_scaling_nz.md): on a large grid a repeating, non-equidistant stack
+    keeps the reciprocity / ky-mirror bank from 16 layers on (the generic class kernel and the class-indexed streaming
+    fallback lose to it); equal thicknesses always take the Toeplitz window kernel or the z-FFT; small grids, where the
+    mirror storage does not apply, deduplicate as before."""
+    def info(nx, ny, dz):
+        plan = hb.plan_create(nx, ny, len(dz), 2.0, 2.0, np.asarray(dz, float), hb.F32)
+        i = hb.plan_info(plan)
+        hb.lib().hfft_destroy(plan)
+        return i
+    alt = lambda nz: [1.0, 2.5] * (nz // 2)
+    for nz in (16, 32, 64):
+        i = info(256, 256, alt(nz))
+        assert (i.dedup, i.mirror) == (0, 3), nz          # symv layout of the reciprocity bank
+    i = info(256, 256, alt(96))
+    assert (i.dedup, i.mirror) == (0, 1)                  # ky-mirror bank (symv: nz <= 64)
+    i = info(256, 256, alt(8))
+    assert i.dedup == 2                                   # generic class kernel, few layers
+    i = info(256, 256, alt(160))
+    assert i.dedup == 1 and i.mirror == 0                 # mirror storage does not fit: class-indexed stream
+    assert info(256, 256, [1.0] * 8).dedup == 3           # Toeplitz window
+    assert info(256, 256, [1.0] * 64).dedup == 4          # z-FFT
+    assert info(256, 256, [1.0] * 128).dedup == 4
+    assert info(32, 32, alt(16)).dedup in (1, 2)          # small grid: deduplicated as before
