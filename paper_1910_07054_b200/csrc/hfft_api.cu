@@ -275,7 +275,7 @@ static void plan_sizes(hfft_plan* p) {
 
 extern "C" {
 
-const char* hfft_version(void) { return "hfft 0.3 sm_100a"; }
+const char* hfft_version(void) { return "hfft 0.4 sm_100a"; }
 
 const char* hfft_last_error(const hfft_plan* plan) { return plan ? plan->error.c_str() : g_create_error.c_str(); }
 
