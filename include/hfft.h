@@ -124,8 +124,10 @@ hfft_status hfft_plan_set_batch(hfft_plan *plan, int batch);
  * (info.bank_bytes shrinks by nz^2 / n_classes) and, where a k-tile of it fits in
  * shared memory, the coupling stage stops being HBM-bound (coupling.cu).
  *   mode 0: off (one slot per pair; required for hfft_update_dz)
- *   mode 1: automatic (default): on when n_classes <= nz^2 / 2; equal thicknesses from 16
- *           layers on use mode 3
+ *   mode 1: automatic (default): a class path is taken where n_classes <= nz^2 / 2 AND it was measured faster
+ *           than the hybrid with its mirror / reciprocity bank: equal thicknesses always (Toeplitz form below 16
+ *           layers, mode 3 from 16 on); other repeating stacks up to 8 layers, and beyond that only where the
+ *           mirror storage does not apply (small grids; nz > 133 in fp32)
  *   mode 2: on (class kernel; Toeplitz form for equal thicknesses)
  *   mode 3: equal thicknesses only: the z-convolution by FFT of PAPER.md:182 Eq.25 as stage S3
  *           (zero-padded transforms of length 2^ceil(log2 2nz) along z at every in-plane
@@ -333,7 +335,7 @@ hfft_status hfft_destroy(hfft_plan *plan);
  * to get the message of the last failing hfft_plan_create on this thread. */
 const char *hfft_last_error(const hfft_plan *plan);
 
-/* Library build identification, e.g. "hfft 0.3 sm_100a". */
+/* Library build identification, e.g. "hfft 0.4 sm_100a". */
 const char *hfft_version(void);
 
 #ifdef __cplusplus
