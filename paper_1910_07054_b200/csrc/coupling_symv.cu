@@ -122,7 +122,7 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     const bool act = w < W;
     const uint32_t smask = s ? 0x80000000u : 0u;             // odd slot = mirror wavevector 2ny - ky: xy, yz change sign
 
-    constexpr uint32_t STAGE = 4 * kSymvCoupleBytes;          // bytes of a full stage
+    constexpr uint32_t STAGE = kSymvStageBytes;               // bytes of a full stage (four couples)
     const uint32_t bars = smem_u32(smem_raw) + warp * (NS * 8);
     const uint32_t ring = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + warp * (NS * STAGE);
     const uint32_t tile = smem_u32(smem_raw) + ((NWARP * NS * 8 + 127) & ~127) + NWARP * NS * STAGE;
@@ -139,7 +139,7 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     // The bookkeeping is kept to a pointer, two counters and one comparison per stage: it runs once per 144 FFMA2.
     const int my_tiles = (int)((n_tiles - blockIdx.x + gridDim.x - 1) / gridDim.x);
     const uint32_t unit_bytes = (uint32_t)G.NC * kSymvCoupleBytes;
-    const int stages_per_unit = (G.NC + 3) >> 2;              // NC = 1 (mod 4): the last stage is one couple
+    const int stages_per_unit = G.SPE;                        // NC = 1 (mod 4): the last stage is one couple
     const long long tile_skip = (long long)gridDim.x * NWARP * unit_bytes - unit_bytes;
     const char* p_ptr = reinterpret_cast<const char*>(bank) + ((long long)blockIdx.x * NWARP + warp) * unit_bytes;
     int p_tiles = my_tiles, p_rep = batch, p_left = stages_per_unit;
@@ -365,7 +365,7 @@ cudaError_t launch_coupling_symv(const CouplingArgs& a, cudaStream_t st) {
     const SymvGeom G = symv_geom(a.nz);
     if (a.tile_k != 2 * NWARP * G.EPW) return cudaErrorInvalidValue;
     auto kern = coupling_symv_kernel<NWARP, NS, MINB>;
-    const size_t smem = ((NWARP * NS * 8 + 127) & ~127) + (size_t)NWARP * NS * 4 * kSymvCoupleBytes +
+    const size_t smem = ((NWARP * NS * 8 + 127) & ~127) + (size_t)NWARP * NS * kSymvStageBytes +
                         (size_t)3 * a.nz * NWARP * G.EPW * 16;
     static PerDevice<int> cache;
     int occ = 1;

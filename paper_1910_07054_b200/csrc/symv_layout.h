@@ -20,7 +20,7 @@
 // float f = 6 h + c of a strip-lane (pair h = 0, 1 of the couple, component c = xx, yy, zz, xy, xz, yz) sits at j = f / 4,
 // element f % 4.  Order of the couples: the full blocks T = 1 .. nfull (column cc = 0..3 of the block: couple 2 cc holds
 // rows 0, 1, couple 2 cc + 1 rows 2, 3), then the half block (4 couples), then T = 0 (5 couples) -- so that every stage
-// of two couples the kernel fetches ends on a block boundary and only the last stage of a unit is short.
+// of four couples (3 KB) the kernel fetches ends on a block boundary and only the last stage of a unit is short (NC = 1 mod 4).
 #pragma once
 
 namespace hfft {
@@ -28,12 +28,12 @@ namespace hfft {
 struct SymvGeom {
     int nz, W, LW, log2LW, EPW, nfull, half;
     int NC;      // couples per unit
-    int SPE;     // stages (two couples; the last one a single couple) per unit
+    int SPE;     // stages (four couples; the last one a single couple) per unit
 };
 
 constexpr int kSymvCoupleFloats = 192;          // 16 strip-lanes x 12 floats
 constexpr int kSymvCoupleBytes = 768;
-constexpr int kSymvStageBytes = 2 * kSymvCoupleBytes;
+constexpr int kSymvStageBytes = 4 * kSymvCoupleBytes;
 constexpr int kSymvMaxNz = 64;                  // 16 strips of 4 rows
 
 __host__ __device__ inline SymvGeom symv_geom(int nz) {
@@ -47,7 +47,7 @@ __host__ __device__ inline SymvGeom symv_geom(int nz) {
     g.nfull = (g.W - 1) / 2;
     g.half = (g.W >= 2 && g.W % 2 == 0) ? 1 : 0;
     g.NC = 8 * g.nfull + 4 * g.half + 5;
-    g.SPE = 4 * g.nfull + 2 * g.half + 3;
+    g.SPE = 2 * g.nfull + g.half + 2;
     return g;
 }
 
