@@ -19,8 +19,9 @@
 // stage with 128-bit shared loads (the two mirror-slot lanes of a strip read the same address: broadcast).
 //
 // M^ / H^ tile.  A CTA of NWARP warps handles TE = NWARP EPW consecutive entries: the [3 nz][2 TE] slots of M^ come in
-// by cp.async (rows of 16 TE bytes), every lane picks up its own 12 values, and H^ goes back through the same shared
-// tile (each lane overwrites exactly the slots it read) and out in full rows.
+// by cp.async (rows of 16 TE bytes) ONE ITEM AHEAD into the other of two tile buffers, every lane picks up its own 12
+// values, and H^ goes back through the same shared tile (each lane overwrites exactly the slots it read) and out in
+// full rows.
 #include <stdint.h>
 
 #include "hfft_internal.h"
@@ -131,8 +132,9 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     // ---- this lane's slots in the M^ / H^ tile: row (c nz + 4 w + r), 16-byte chunk el ^ swizzle(w), half s ----
     const int el = warp * EPW + ent;
     const int chunk = el ^ ((w * EPW) & (TE - 1));
-    const uint32_t my_slot = tile + (uint32_t)chunk * 16 + (uint32_t)s * 8;
+    const uint32_t my_off = (uint32_t)chunk * 16 + (uint32_t)s * 8;
     const uint32_t row_bytes = (uint32_t)TE * 16;
+    const uint32_t tile_bytes = (uint32_t)(3 * nz) * row_bytes;     // two tile buffers: the next item's M^ arrives while this one is worked on
 
     // ---- bank ring: producer state (uniform over the warp; lane 0 issues) ----
     // this CTA's tiles: blockIdx.x, blockIdx.x + gridDim.x, ...; every tile is streamed once per state of the batch.
@@ -190,20 +192,30 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
     const int log2TE = 3 + 4 - G.log2LW;                     // TE = NWARP EPW = 8 * 16 / LW
     static_assert(NWARP == 8, "log2TE assumes 8 warps per CTA");
     const int chunks_per_tile = np << log2TE;
-    for (int it = 0; it < my_tiles; ++it)
-    for (int b = 0; b < batch; ++b) {
+    const int n_items = my_tiles * batch;
+    // M^ tile of item n into buffer buf: rows of 16 TE bytes, chunk index swizzled by the strip of the row's layer
+    auto fetch = [&](int n, int buf) {
+        const int it = n / batch, b = n - it * batch;
         const long long t = blockIdx.x + (long long)it * gridDim.x;
-        float2* sp = spec + (long long)b * np * ks + t * (2 * TE);
-
-        // ---- M^ tile in: rows of 16 TE bytes, chunk index swizzled by the strip of the row's layer ----
+        const float2* sp = spec + (long long)b * np * ks + t * (2 * TE);
+        const uint32_t dst = tile + buf * tile_bytes;
         for (int x = tid; x < chunks_per_tile; x += 32 * NWARP) {
             const int lp = x >> log2TE, ch = x & (TE - 1);
             const int layer = lp - (lp >= 2 * nz ? 2 * nz : (lp >= nz ? nz : 0));
             const int chs = ch ^ (((layer >> 2) * EPW) & (TE - 1));
-            cp_async16(tile + (uint32_t)lp * row_bytes + (uint32_t)chs * 16, sp + (long long)lp * ks + ch * 2);
+            cp_async16(dst + (uint32_t)lp * row_bytes + (uint32_t)chs * 16, sp + (long long)lp * ks + ch * 2);
         }
+    };
+    if (n_items > 0) fetch(0, 0);
+    for (int n = 0; n < n_items; ++n) {
+        const int it = n / batch, b = n - it * batch;
+        const long long t = blockIdx.x + (long long)it * gridDim.x;
+        float2* sp = spec + (long long)b * np * ks + t * (2 * TE);
         cp_async_wait_all();
-        __syncthreads();
+        __syncthreads();                                     // this item's M^ has landed; the other buffer's H^ has been copied out
+        if (n + 1 < n_items) fetch(n + 1, (n + 1) & 1);      // a different k range of the in-place spectrum: no hazard with this item's H^
+        const uint32_t tbuf = tile + (n & 1) * tile_bytes;
+        const uint32_t my_slot = tbuf + my_off;
 
         float2 mp[4][3], hp[4][3];
 #pragma unroll
@@ -344,10 +356,9 @@ coupling_symv_kernel(const float* __restrict__ bank, float2* __restrict__ spec, 
             const int lp = x >> log2TE, ch = x & (TE - 1);
             const int layer = lp - (lp >= 2 * nz ? 2 * nz : (lp >= nz ? nz : 0));
             const int chs = ch ^ (((layer >> 2) * EPW) & (TE - 1));
-            const float4 v = lds128(tile + (uint32_t)lp * row_bytes + (uint32_t)chs * 16);
+            const float4 v = lds128(tbuf + (uint32_t)lp * row_bytes + (uint32_t)chs * 16);
             *reinterpret_cast<float4*>(sp + (long long)lp * ks + ch * 2) = v;
         }
-        __syncthreads();                                     // the tile is free for the next item's cp.async
     }
 }
 
@@ -366,7 +377,7 @@ cudaError_t launch_coupling_symv(const CouplingArgs& a, cudaStream_t st) {
     if (a.tile_k != 2 * NWARP * G.EPW) return cudaErrorInvalidValue;
     auto kern = coupling_symv_kernel<NWARP, NS, MINB>;
     const size_t smem = ((NWARP * NS * 8 + 127) & ~127) + (size_t)NWARP * NS * kSymvStageBytes +
-                        (size_t)3 * a.nz * NWARP * G.EPW * 16;
+                        (size_t)2 * 3 * a.nz * NWARP * G.EPW * 16;
     static PerDevice<int> cache;
     int occ = 1;
     cudaError_t err = ctas_per_sm_cached(kern, 32 * NWARP, smem, cache, occ);
