@@ -15,8 +15,9 @@
 //     S^c(kz) = [         2 sum_{d>0} a^c_d sin(2 pi kz d / Lz) ] / Lz      c = xz, yz   (i * (-i) = 1)
 // all real: H^(k, kz) = S(k, kz) M^(k, kz) with S the symmetric matrix [[xx,xy,xz],[xy,yy,yz],[xz,yz,zz]]
 // acting on the UNROTATED spectra (S2 / S4 run with nz_rot = 0 in this mode).
-// Layout [tile][kz][6][32] in the plan precision: every value is read once per evaluation, straight
-// from global memory (128 B per warp), 6 Lz reals per wavevector.
+// The cosine sums are even in kz and the sine sums odd, S^c(Lz - kz) = +- S^c(kz), so only kz = 0 .. Lz / 2 is stored:
+// layout [tile][kz <= Lz/2][6][32] in the plan precision, 6 (Lz / 2 + 1) reals per wavevector, every value read once
+// per evaluation (128 B per warp); kz > Lz / 2 uses slot Lz - kz with xz, yz negated.
 //
 // Kernel: lane = wavevector (global accesses are 256 B per warp along k), warp t of the TT warps of
 // a CTA owns the layers n = t + TT q, q < E (Lz = E TT).  Forward (decimation in frequency):
@@ -74,17 +75,19 @@ template <typename T, int LOG2LZ> struct ZOcc {
     static constexpr int LZ = ZCfg<LOG2LZ>::LZ, TT = ZCfg<LOG2LZ>::TT;
     static constexpr int THREADS = 32 * TT;
     static constexpr size_t EX_BYTES = TT > 1 ? (size_t)3 * LZ * 32 * sizeof(C) : 0;
-    static constexpr size_t BANK_BYTES = (size_t)LZ * 6 * 32 * sizeof(T);
+    static constexpr size_t BANK_BYTES = (size_t)(LZ / 2 + 1) * 6 * 32 * sizeof(T);   // kz = 0 .. LZ / 2
     static constexpr bool STAGE = TT > 1 && EX_BYTES + BANK_BYTES + LZ * sizeof(C) <= 200 * 1024;
     static constexpr size_t SMEM = EX_BYTES + (STAGE ? BANK_BYTES : 0) + LZ * sizeof(C);
 };
 
-// multiply the three components at one (k, kz) by the real symmetric S(k, kz); bt: shared or global
+// multiply the three components at one (k, kz) by the real symmetric S(k, kz); bt: shared or global, slot of
+// min(kz, LZ - kz); neg: kz > LZ / 2, the odd components xz, yz change sign
 template <bool SMEM, typename T, typename C>
-__device__ __forceinline__ void zmul(const T* __restrict__ bt, C& x, C& y, C& z) {
+__device__ __forceinline__ void zmul(const T* __restrict__ bt, bool neg, C& x, C& y, C& z) {
     T a[6];
 #pragma unroll
     for (int c = 0; c < 6; ++c) a[c] = SMEM ? bt[c * 32] : __ldcs(bt + c * 32);
+    if (neg) { a[4] = -a[4]; a[5] = -a[5]; }
     const C mx = x, my = y, mz = z;
     C hx = cscale(a[0], mx), hy = cscale(a[3], mx), hz = cscale(a[4], mx);
     hx = caxpy(a[3], my, hx); hy = caxpy(a[1], my, hy); hz = caxpy(a[5], my, hz);
@@ -104,7 +107,7 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
     constexpr int CHUNK_T = 16 / sizeof(T);
     extern __shared__ __align__(16) unsigned char smem_raw[];
     C* ex = reinterpret_cast<C*>(smem_raw);                                   // [3][LZ][32] (TT > 1)
-    T* sbank = reinterpret_cast<T*>(smem_raw + O::EX_BYTES);                   // [LZ][6][32] (STAGE)
+    T* sbank = reinterpret_cast<T*>(smem_raw + O::EX_BYTES);                   // [LZ / 2 + 1][6][32] (STAGE)
     C* stw = reinterpret_cast<C*>(smem_raw + O::EX_BYTES + (STAGE ? O::BANK_BYTES : 0));   // [LZ] exp(-2 pi i n / LZ)
     const int lane = threadIdx.x & 31, t = threadIdx.x >> 5;
     const int np = 3 * nz;
@@ -113,8 +116,8 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
     const long long n_items = n_tiles * batch;
     auto fetch_bank = [&](long long it) {
         if (STAGE && it < n_items) {
-            const T* src = bank3 + (it / batch) * LZ * (6LL * TK);
-            for (int x = threadIdx.x; x < LZ * 6 * TK / CHUNK_T; x += blockDim.x)
+            const T* src = bank3 + (it / batch) * (LZ / 2 + 1) * (6LL * TK);
+            for (int x = threadIdx.x; x < (LZ / 2 + 1) * 6 * TK / CHUNK_T; x += blockDim.x)
                 cp_async16(sbank + x * CHUNK_T, src + x * CHUNK_T);
         }
         cp_async_commit();
@@ -163,14 +166,15 @@ coupling_zfft_kernel(const T* __restrict__ bank3, HFFT_C* __restrict__ spec, con
                 for (int rr = 0; rr < RPT; ++rr) rdft<TT, false, false, T>(&v[c][rr * TT]);
         }
         // ---- v[c][rr TT + s] = M^_c(k, kz), kz = r + E s, r = t RPT + rr: multiply by S(k, kz) ----
-        const T* bt = STAGE ? sbank + lane : bank3 + tile * LZ * (6LL * TK) + lane;
+        const T* bt = STAGE ? sbank + lane : bank3 + tile * (LZ / 2 + 1) * (6LL * TK) + lane;
 #pragma unroll
         for (int rr = 0; rr < RPT; ++rr)
 #pragma unroll
             for (int s = 0; s < TT; ++s) {
                 const int kz = (TT > 1 ? t * RPT + rr : rr) + E * s;
                 const int o = rr * TT + s;
-                zmul<STAGE, T>(bt + kz * 6 * TK, v[0][o], v[1][o], v[2][o]);
+                const bool neg = kz > LZ / 2;
+                zmul<STAGE, T>(bt + (neg ? LZ - kz : kz) * 6 * TK, neg, v[0][o], v[1][o], v[2][o]);
             }
         // ---- inverse ----
         if constexpr (TT > 1) {
@@ -251,7 +255,7 @@ coupling_zfft2_kernel(const float* __restrict__ bank3, float2* __restrict__ spec
         const long long tile = item / batch;
         const int b = (int)(item - tile * batch);
         C* sp = spec + (long long)b * np * ks + tile * TK + lane;
-        const T* bt = bank3 + tile * LZ * (6LL * TK) + lane;
+        const T* bt = bank3 + tile * (LZ / 2 + 1) * (6LL * TK) + lane;            // slots kz = 0 .. LZ / 2
         // ---- forward, first stage: DFT_E over q (upper half zero), twiddle W_LZ^{t r}; all loads first ----
         {
             C in[3][E / 2];
@@ -283,9 +287,11 @@ coupling_zfft2_kernel(const float* __restrict__ bank3, float2* __restrict__ spec
                 constexpr int HS = TT / 2;                   // S values in two batches: 24 registers at a time
                 T a[HS][6];
 #pragma unroll
-                for (int s = 0; s < HS; ++s)
+                for (int s = 0; s < HS; ++s) {
+                    const int kz = r + E * s, kzh = kz > LZ / 2 ? LZ - kz : kz;
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * s) * 6 + c) * TK);
+                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + (kzh * 6 + c) * TK);
+                }
                 C w[3][TT];
 #pragma unroll
                 for (int c = 0; c < 3; ++c) {
@@ -298,17 +304,22 @@ coupling_zfft2_kernel(const float* __restrict__ bank3, float2* __restrict__ spec
 #pragma unroll
                     for (int s = 0; s < HS; ++s) {           // kz = r + E (half HS + s)
                         const int o = half * HS + s;
-                        const C mx = w[0][o], my = w[1][o], mz = w[2][o];
+                        // kz > LZ / 2: S(kz) = D S(LZ - kz) D, D = diag(1, 1, -1) -- the sign goes on M_z and H_z (values
+                        // already here), not on the S values still in flight
+                        const T sg = (r + E * o) > LZ / 2 ? (T)-1 : (T)1;
+                        const C mx = w[0][o], my = w[1][o], mz = cscale(sg, w[2][o]);
                         C hx = cscale(a[s][0], mx), hy = cscale(a[s][3], mx), hz = cscale(a[s][4], mx);
                         hx = caxpy(a[s][3], my, hx); hy = caxpy(a[s][1], my, hy); hz = caxpy(a[s][5], my, hz);
                         hx = caxpy(a[s][4], mz, hx); hy = caxpy(a[s][5], mz, hy); hz = caxpy(a[s][2], mz, hz);
-                        w[0][o] = hx; w[1][o] = hy; w[2][o] = hz;
+                        w[0][o] = hx; w[1][o] = hy; w[2][o] = cscale(sg, hz);
                     }
                     if (half == 0) {
 #pragma unroll
-                        for (int s = 0; s < HS; ++s)
+                        for (int s = 0; s < HS; ++s) {
+                            const int kz = r + E * (HS + s), kzh = kz > LZ / 2 ? LZ - kz : kz;
 #pragma unroll
-                            for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * (HS + s)) * 6 + c) * TK);
+                            for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + (kzh * 6 + c) * TK);
+                        }
                     }
                 }
 #pragma unroll
@@ -334,17 +345,20 @@ coupling_zfft2_kernel(const float* __restrict__ bank3, float2* __restrict__ spec
             for (int s0 = 0; s0 < TT; s0 += 4) {
                 T a[4][6];
 #pragma unroll
-                for (int s = 0; s < 4; ++s)
+                for (int s = 0; s < 4; ++s) {
+                    const int kz = r + E * (s0 + s), kzh = kz > LZ / 2 ? LZ - kz : kz;
 #pragma unroll
-                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + ((r + E * (s0 + s)) * 6 + c) * TK);
+                    for (int c = 0; c < 6; ++c) a[s][c] = __ldcs(bt + (kzh * 6 + c) * TK);
+                }
 #pragma unroll
                 for (int s = 0; s < 4; ++s) {
                     C* e0 = ex + (r * TT + s0 + s) * TK + lane;
-                    const C mx = e0[0], my = e0[LZ * TK], mz = e0[2 * LZ * TK];
+                    const T sg = (r + E * (s0 + s)) > LZ / 2 ? (T)-1 : (T)1;     // S(kz) = D S(LZ - kz) D, D = diag(1, 1, -1)
+                    const C mx = e0[0], my = e0[LZ * TK], mz = cscale(sg, e0[2 * LZ * TK]);
                     C hx = cscale(a[s][0], mx), hy = cscale(a[s][3], mx), hz = cscale(a[s][4], mx);
                     hx = caxpy(a[s][3], my, hx); hy = caxpy(a[s][1], my, hy); hz = caxpy(a[s][5], my, hz);
                     hx = caxpy(a[s][4], mz, hx); hy = caxpy(a[s][5], mz, hy); hz = caxpy(a[s][2], mz, hz);
-                    e0[0] = hx; e0[LZ * TK] = hy; e0[2 * LZ * TK] = hz;
+                    e0[0] = hx; e0[LZ * TK] = hy; e0[2 * LZ * TK] = cscale(sg, hz);
                 }
             }
 #pragma unroll 1
@@ -416,13 +430,13 @@ zdft_bank_kernel(T* __restrict__ bank3, const double* __restrict__ cls64, const 
     const long long tile = k / 32;
     const int kk = (int)(k - tile * 32);
 #pragma unroll
-    for (int c = 0; c < 6; ++c) bank3[((tile * LZ + kz) * 6 + c) * 32 + kk] = (T)(acc[c] / LZ);
+    for (int c = 0; c < 6; ++c) bank3[((tile * (LZ / 2 + 1) + kz) * 6 + c) * 32 + kk] = (T)(acc[c] / LZ);   // kz <= LZ / 2
 }
 
 cudaError_t launch_zdft_bank(void* bank3, const double* cls64, const void* twz64, int nz, int log2lz, long long n_k,
                              long long kstride, long long n_k_padded, int prec, cudaStream_t st) {
     const int LZ = 1 << log2lz;
-    dim3 grid((unsigned)((n_k_padded + 127) / 128), LZ);
+    dim3 grid((unsigned)((n_k_padded + 127) / 128), LZ / 2 + 1);          // S(LZ - kz) = +- S(kz): kz = 0 .. LZ / 2 only
     if (prec == HFFT_F32)
         zdft_bank_kernel<float><<<grid, 128, 0, st>>>((float*)bank3, cls64, (const double2*)twz64, nz, LZ, n_k, kstride,
                                                       n_k_padded);

@@ -260,7 +260,7 @@ static void plan_sizes(hfft_plan* p) {
     p->n_slots = p->mirror ? (long long)(p->nx + 1) * (2 * p->ny + 2) : p->n_k;
     p->n_tiles = (p->n_slots + p->tile_k - 1) / p->tile_k;
     p->n_k_padded = p->n_tiles * p->tile_k;
-    const size_t slots = p->zfft ? ((size_t)1 << p->log2lz)
+    const size_t slots = p->zfft ? (((size_t)1 << p->log2lz) / 2 + 1)          // S(k, kz), kz = 0 .. Lz / 2 (coupling_zfft.cu)
                          : (p->recip ? (size_t)p->nz * (p->nz + 1) / 2 : (p->dedup ? p->n_classes : p->nz * p->nz));
     p->bank_bytes = (size_t)6 * slots * (size_t)(p->mirror ? p->n_k_padded / 2 : p->n_k_padded) * e;
     if (p->symv) p->bank_bytes = coupling_symv_bank_bytes(p->nz, p->n_tiles);
