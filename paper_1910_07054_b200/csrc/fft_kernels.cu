@@ -143,12 +143,15 @@ fftx_fwd_kernel(const T* __restrict__ in, HFFT_C* __restrict__ xhat, int log2rb,
 // and the sum of m h over the plane's cells (doubles, one atomicAdd per warp and block) into
 // sums[plane][2] -- the layer average <H_z> of PAPER.md:209 and the m.H sums of the demagnetization energy.
 template <typename T, int LOG2N, bool RED>
-__global__ void __launch_bounds__(XCfg<T>::MAXT, XCfg<T>::MINB)
+__global__ void __launch_bounds__(XCfg<T>::MAXT, 1)
 ifftx_kernel(const HFFT_C* __restrict__ xhat, T* __restrict__ out, int log2rb, int rows_per_plane,
              const HFFT_C* __restrict__ tw, const HFFT_C* __restrict__ twt, long long nblocks, int bpc,
              const T* __restrict__ m, double* __restrict__ sums) {
     typedef HFFT_C C;
-    typedef RowFFT<T, LOG2N, true, false, false> F;
+    // fp32: twiddles in registers and one 512-thread CTA per SM (112-122 registers) -- measured against table twiddles
+    // with two CTAs per SM (64 registers): C5 S5 0.712 -> 0.672 ms, C3 0.0178 -> 0.0167 ms, C4 0.0516 -> 0.0505 ms; the
+    // same change does nothing for S1 (C5 0.700 -> 0.716 ms), which keeps the table
+    typedef RowFFT<T, LOG2N, true, false, sizeof(T) == 4> F;
     constexpr int N = F::N, R = F::R, TPR = F::TPR, SH = F::SH;
     constexpr int IT = R > 1 ? R / 2 : 1;
     constexpr int RS = R > 1 ? R / 2 : 1;                    // stores per thread (crop)
