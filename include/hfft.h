@@ -294,6 +294,55 @@ hfft_status hfft_host_join(hfft_plan *plan, void *stream);
 hfft_status hfft_update_dz(hfft_plan *plan, int k, double dz_new, void *stream);
 
 /*
+ * hfft_update_dz for callers that must not allocate device memory.
+ *
+ * Who this is for.  hfft_update_dz takes its setup scratch (info.setup_scratch_bytes) from
+ * cudaMalloc and gives it back with cudaFree on EVERY call.  That is not possible for
+ *   - a simulation code that has handed all of the GPU's memory to a pool of its own at start-up
+ *     (a framework's caching allocator, a pre-sized arena): cudaMalloc then fails with "out of
+ *     memory" although the program has room to spare;
+ *   - a thickness-optimisation or real-time loop (PAPER.md:205-211 rebuilds the tensor at every
+ *     Newton step) that cannot accept what cudaMalloc / cudaFree bring with them: a device-wide
+ *     synchronisation, a driver lock, a run time that nobody bounds;
+ *   - a host thread that works while another thread of the process records a CUDA graph in the
+ *     global capture mode, where cudaMalloc is a forbidden call and breaks the recording.
+ * This entry point does the same work -- same arguments, same kernels, same arithmetic, the bank
+ * comes out bit for bit as from hfft_update_dz -- but its scratch is a fixed array that lives in
+ * the library's device image.  It calls no cudaMalloc, no cudaFree and no library routine that
+ * allocates device memory (on the host it uses a few small std::vector tables, as hfft_update_dz does).
+ *
+ * The limit.  The array has HFFT_STATIC_SCRATCH_BYTES = 32 MiB.  A plan whose
+ * info.setup_scratch_bytes is larger is refused with HFFT_EUNSUPPORTED and a message that gives
+ * both numbers; nothing has been touched then.  32 MiB holds e.g. 64 x 64 cells with up to 8
+ * layers or 32 x 32 with up to 32 (the paper's 60 nm disc example, 64 x 64 x 5, needs 19 MB).
+ * Larger plans use hfft_update_dz.
+ *
+ * What it costs.  Every GPU on which the CUDA runtime loads this part of the library holds the
+ * 32 MiB from that moment -- at the latest the first call of this function on that GPU -- until the
+ * process exits; hfft_destroy does not release it.
+ *
+ * First call on a device.  The first call made while a given device is current looks up the
+ * array's address on that device (cudaGetSymbolAddress, which also makes the runtime load the
+ * device image) and keeps it.  Make that first call at start-up, before any stream capture begins
+ * anywhere in the process; later calls only read the stored address.
+ *
+ * Sharing.  All plans and all host threads of the process use the same array on a device, and it
+ * keeps whatever the previous call left in it.  Nothing in the rebuild relies on old contents:
+ * the one region that has to start at zero (the padded real-space tensor planes) is cleared on
+ * the stream at the start of every call.  Two rebuilds running on the GPU at the same time would
+ * overwrite each other's intermediate results and leave wrong banks without any error.  The
+ * library keeps that from happening inside one process: the call holds a lock from its first
+ * enqueue until it has synchronised `stream`, so a second caller waits.  Do not defeat it (for
+ * instance by calling from a host callback of the same stream).
+ *
+ * Otherwise as hfft_update_dz: enqueues on `stream`, synchronises it before returning, commits
+ * dz[k] only when the rebuild went through.  Errors: those of hfft_update_dz except ENOMEM, plus
+ * EUNSUPPORTED for a plan beyond the limit.
+ */
+#define HFFT_STATIC_SCRATCH_BYTES (32u * 1024u * 1024u)
+hfft_status hfft_update_dz_static(hfft_plan *plan, int k, double dz_new, void *stream);
+
+/*
  * Fused reductions of the field.  With a non-NULL
  * `sums_device` (DEVICE pointer to B*3*nz*2 doubles, caller-owned, 8-byte
  * aligned) every following hfft_demag / hfft_demag_host zeroes that array and

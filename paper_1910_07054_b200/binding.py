@@ -21,11 +21,12 @@ STATUS_NAMES = ["HFFT_OK", "HFFT_EINVAL", "HFFT_ENOMEM", "HFFT_ECUDA", "HFFT_EST
 NUM_STAGES = 5
 STAGE_NAMES = ["fftx_fwd", "ffty_fwd", "coupling", "iffty", "ifftx"]
 MAX_NZ = 256
+STATIC_SCRATCH_BYTES = 32 * 1024 * 1024
 
 # every symbol include/hfft.h declares
 EXPORTS = ["hfft_plan_create", "hfft_plan_set_batch", "hfft_plan_set_dedup", "hfft_plan_set_mirror", "hfft_plan_set_recip", "hfft_plan_set_fusion",
            "hfft_tensor_classes", "hfft_plan_info", "hfft_bank_bytes", "hfft_workspace_bytes", "hfft_plan_set_buffers",
-           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_plan_set_reduction",
+           "hfft_build_tensor", "hfft_demag", "hfft_demag_host", "hfft_demag_host_async", "hfft_host_join", "hfft_update_dz", "hfft_update_dz_static", "hfft_plan_set_reduction",
            "hfft_profile_enable", "hfft_profile_read",
            "hfft_read_bank", "hfft_destroy", "hfft_last_error", "hfft_version"]
 
@@ -77,6 +78,7 @@ def lib():
         L.hfft_demag_host_async.argtypes = [vp, vp, dp, vp, vp]
         L.hfft_host_join.argtypes = [vp, vp]
         L.hfft_update_dz.argtypes = [vp, ctypes.c_int, ctypes.c_double, vp]
+        L.hfft_update_dz_static.argtypes = [vp, ctypes.c_int, ctypes.c_double, vp]
         L.hfft_plan_set_reduction.argtypes = [vp, vp]
         L.hfft_profile_enable.argtypes = [vp, ctypes.c_int]
         L.hfft_profile_read.argtypes = [vp, dp, ip]
@@ -215,6 +217,12 @@ def update_dz(plan, k, dz_new, stream=0):
     _check(lib().hfft_update_dz(plan, int(k), float(dz_new), ctypes.c_void_p(stream)), plan)
 
 
+def update_dz_static(plan, k, dz_new, stream=0):
+    """hfft_update_dz_static: the same rebuild with its scratch in the library's fixed 32 MiB device array
+    (STATIC_SCRATCH_BYTES) instead of cudaMalloc / cudaFree -- for callers that must not allocate."""
+    _check(lib().hfft_update_dz_static(plan, int(k), float(dz_new), ctypes.c_void_p(stream)), plan)
+
+
 def plan_set_reduction(plan, sums_ptr):
     """sums_ptr: device address of B*3*nz*2 doubles, or 0 / None to switch the reductions off."""
     _check(lib().hfft_plan_set_reduction(plan, ctypes.c_void_p(sums_ptr or None)), plan)
@@ -316,6 +324,9 @@ class Plan:
 
     def update_dz(self, k, dz_new):
         update_dz(self.handle, k, dz_new, self._stream())
+
+    def update_dz_static(self, k, dz_new):
+        update_dz_static(self.handle, k, dz_new, self._stream())
 
     def set_reduction(self, on=True):
         """Returns the device tensor [B][3][nz][2] = (sum of h_c, sum of m_c h_c) per plane that every

@@ -68,6 +68,31 @@ struct hfft_plan {
     std::string error;
 };
 
+// ---- scratch of hfft_update_dz_static (hfft.h) ----
+// A fixed array in this translation unit's device image: it exists on every device that loads the image and is never
+// freed.  In HOST code the name below is only a handle for the runtime, not a device address -- a kernel handed
+// `g_static_scratch` itself would fault (or, where the GPU can reach host memory, quietly work on the wrong bytes).
+// The address that kernels can use comes from cudaGetSymbolAddress, asked once per device with that device current.
+static __device__ __align__(256) unsigned char g_static_scratch[HFFT_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxCachedDevices = 64;
+std::mutex g_static_mu;                                  // held for a whole hfft_update_dz_static call
+void* g_static_addr[kMaxCachedDevices] = {};             // device ordinal -> address of g_static_scratch there
+
+// Device address of the scratch array on the CURRENT device `dev`; g_static_mu must be held.
+cudaError_t static_scratch_address(int dev, void** out) {
+    if (dev >= 0 && dev < kMaxCachedDevices && g_static_addr[dev]) { *out = g_static_addr[dev]; return cudaSuccess; }
+    void* ptr = nullptr;
+    cudaError_t e = cudaGetSymbolAddress(&ptr, g_static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!ptr || ((size_t)ptr & 255)) return cudaErrorInvalidSymbol;
+    if (dev >= 0 && dev < kMaxCachedDevices) g_static_addr[dev] = ptr;
+    *out = ptr;
+    return cudaSuccess;
+}
+}  // namespace
+
 static hfft_status fail(hfft_plan* p, hfft_status s, const std::string& msg) {
     if (p) p->error = msg; else g_create_error = msg;
     return s;
@@ -608,6 +633,54 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
         return fail_cuda(plan, "hfft_update_dz: cudaStreamSynchronize", e2);
     }
     // the tensor classes of the new stack (hfft_plan_info.n_classes; the bank itself is not deduplicated here)
+    pair_classes(plan->nz, plan->dz.data(), plan->pair_class, plan->class_rep, plan->toeplitz);
+    plan->n_classes = (int)plan->class_rep.size();
+    return HFFT_OK;
+}
+
+// hfft_update_dz without device allocation (hfft.h): the rebuild of hfft_update_dz with its scratch in g_static_scratch.
+// The existing function is left as it is; this one repeats its few lines of orchestration.
+hfft_status hfft_update_dz_static(hfft_plan* plan, int k, double dz_new, void* stream) {
+    if (!plan) return HFFT_EINVAL;
+    if (k < 0 || k >= plan->nz) return fail(plan, HFFT_EINVAL, "hfft_update_dz_static: layer index out of range");
+    if (!(dz_new > 0) || !isfinite(dz_new)) return fail(plan, HFFT_EINVAL, "hfft_update_dz_static: dz must be positive and finite");
+    if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_update_dz_static: call hfft_build_tensor first");
+    if (plan->dedup)
+        return fail(plan, HFFT_EUNSUPPORTED, "hfft_update_dz_static: the bank is deduplicated; create the plan with hfft_plan_set_dedup(plan, 0)");
+    if (plan->recip && !plan->d_invdz) return fail(plan, HFFT_ESTATE, "hfft_update_dz_static: 1/dz table missing; rebuild the plan");
+    // the size depends on the grid and the layer count only, not on the thicknesses: check it before anything changes
+    {
+        const size_t need = build_scratch_bytes(make_geom(plan));
+        if (need > (size_t)HFFT_STATIC_SCRATCH_BYTES)
+            return fail(plan, HFFT_EUNSUPPORTED,
+                        "hfft_update_dz_static: this plan needs " + std::to_string(need) + " bytes of setup scratch, the fixed array holds " +
+                            std::to_string((size_t)HFFT_STATIC_SCRATCH_BYTES) + " (HFFT_STATIC_SCRATCH_BYTES); use hfft_update_dz");
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
+    // one rebuild at a time per process: the array is shared by every plan and thread, and the call below ends with
+    // a synchronisation of `st`, so nothing of this call is still running when the lock is released
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    void* scratch = nullptr;
+    if ((e = static_scratch_address(plan->device, &scratch)) != cudaSuccess)
+        return fail_cuda(plan, "hfft_update_dz_static: cudaGetSymbolAddress(static scratch)", e);
+    const double dz_old = plan->dz[k];
+    plan->dz[k] = dz_new;
+    BuildGeom g = make_geom(plan);
+    std::string msg;
+    // The array still holds the previous call's intermediates.  build_bank writes every table it reads (interface
+    // coordinates, class table, lattice and stencil values, transforms) and clears, on `st`, the real-space planes
+    // whose padding must be zero -- the same as with the uninitialised memory cudaMalloc hands out.
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, plan->recip ? -1 : k, st, msg);
+    if (e == cudaSuccess && plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) msg = "1/dz table";   // d_invdz exists: a copy only
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    if (e != cudaSuccess || e2 != cudaSuccess) {
+        plan->dz[k] = dz_old;
+        plan->built = false;
+        if (e != cudaSuccess) return fail(plan, HFFT_ECUDA, "hfft_update_dz_static: " + msg);
+        return fail_cuda(plan, "hfft_update_dz_static: cudaStreamSynchronize", e2);
+    }
     pair_classes(plan->nz, plan->dz.data(), plan->pair_class, plan->class_rep, plan->toeplitz);
     plan->n_classes = (int)plan->class_rep.size();
     return HFFT_OK;
