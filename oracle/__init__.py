@@ -11,6 +11,7 @@ from .oracle import (  # noqa: F401
     tensor_point,
     nxx_fp64,
     tensor_row,
+    tensor_spectrum,
     direct_field,
     direct_cells,
     hybrid_field,

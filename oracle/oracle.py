@@ -199,7 +199,22 @@ def _pad_kernel(Nrow, nx, ny):
     return pad
 
 
-def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive", rows=None):
+def tensor_spectrum(Nrow, nx, ny, dft="naive"):
+    """Left factor of Eq.24, F1F2(N_kl) of one target layer: the tensor row placed on the
+    2nx x 2ny periodic grid (A10) and transformed in the plane.  Nrow: tensor_row(..., i); returns complex
+    [nz][6][2ny][2nx].  These are the lines hybrid_layers runs per target layer, under a name of their own so that a
+    caller (bench.py's CPU baseline: "tensor bank pre-built, setup excluded, as for the GPU") can run them once,
+    outside its timing, and hand the result back through `nhat=`."""
+    pad = _pad_kernel(Nrow, nx, ny)
+    if dft == "naive":
+        Wx, Wy = _dft_matrix(2 * nx), _dft_matrix(2 * ny)
+        return np.einsum("kq,jcqp,np->jckn", Wy, pad, Wx, optimize=True)
+    if dft == "fft":
+        return np.fft.fft2(pad, axes=(-2, -1))
+    raise ValueError(dft)
+
+
+def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive", rows=None, nhat=None):
     """T1: Eq.24 for the listed target layers.
 
       H_{k,i1,i2,i3} = - sum_l F2^-1 F1^-1 sum_{j3} [ F1F2(N_kl)_{i3-j3} F1F2(M_l)_{j3} ]_{i1,i2}
@@ -209,6 +224,8 @@ def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive", rows=None)
     Returns [len(layers)][3][ny][nx] (or [B][len(layers)][3][ny][nx]).
     rows: optional {i: tensor_row(..., i)} of precomputed tensor rows (setup hoisted out, e.g. when
     bench.py times the evaluation without the tensor build); the arithmetic is unchanged.
+    nhat: optional {i: tensor_spectrum(rows[i], nx, ny, dft)} of precomputed tensor spectra -- the same hoist one step
+    further (the GPU path's hfft_build_tensor covers both); the arithmetic is unchanged.
     """
     M = _magnetisation(m, Ms, nz)
     batched = M.ndim == 5
@@ -226,14 +243,12 @@ def hybrid_layers(nx, ny, nz, dx, dy, dz, m, Ms, layers, dft="naive", rows=None)
         raise ValueError(dft)
     out = np.empty((B, len(layers), 3, ny, nx))
     for t, i in enumerate(layers):
-        Nrow = rows[i] if rows is not None and i in rows else tensor_row(nx, ny, nz, dx, dy, dz, i)
-        pad = _pad_kernel(Nrow, nx, ny)
-        del Nrow
-        if dft == "naive":
-            Nhat = np.einsum("kq,jcqp,np->jckn", Wy, pad, Wx, optimize=True)
+        if nhat is not None and i in nhat:
+            Nhat = nhat[i]
         else:
-            Nhat = np.fft.fft2(pad, axes=(-2, -1))
-        del pad
+            Nrow = rows[i] if rows is not None and i in rows else tensor_row(nx, ny, nz, dx, dy, dz, i)
+            Nhat = tensor_spectrum(Nrow, nx, ny, dft)
+            del Nrow
         for k in range(3):
             Hhat = np.zeros((B, 2 * ny, 2 * nx), dtype=np.complex128)
             for l in range(3):

@@ -59,6 +59,26 @@ def test_naive_dft_equals_fft_and_batched():
         assert _relerr(Hn[b], H0) < 1e-14
 
 
+@pytest.mark.parametrize("dft", ["naive", "fft"])
+def test_hoisted_setup_arguments_do_not_change_the_field(dft):
+    """hybrid_layers(rows=, nhat=): tensor rows / tensor spectra computed by the caller beforehand (what bench.py's CPU
+    baseline does so that it times the evaluation with the bank pre-built, like the GPU arm) give the same bits as
+    the call that computes them itself, and the spectrum they carry is the DFT of the periodic tensor (checked at
+    k = 0, where the transform is the plain sum over the offsets)."""
+    w = W.small(8, 4, 3, B=2, seed=9)
+    m = w.m()
+    layers = [2, 0]
+    plain = O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, layers, dft=dft)
+    rows = {i: O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, i) for i in layers}
+    nhat = {i: O.tensor_spectrum(rows[i], w.nx, w.ny, dft) for i in layers}
+    assert nhat[0].shape == (w.nz, 6, 2 * w.ny, 2 * w.nx)
+    assert np.abs(nhat[2][:, :, 0, 0] - rows[2].sum(axis=(-1, -2))).max() <= 1e-14 * np.abs(rows[2]).sum(axis=(-1, -2)).max()
+    assert np.array_equal(O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, layers, dft=dft, rows=rows), plain)
+    assert np.array_equal(O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, layers, dft=dft, nhat=nhat), plain)
+    # a partial dictionary falls back to the computation for the missing layer
+    assert np.array_equal(O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, layers, dft=dft, nhat={0: nhat[0]}), plain)
+
+
 def test_linearity_in_per_layer_Ms():
     w = W.small(8, 8, 3, seed=4)
     m = w.m()[0]
