@@ -97,54 +97,116 @@ def algorithmic_bytes(w, n_slots=None, mirror=False, recip=False, fused=False):
 
 
 class ClockSampler:
+    """SM clock and throttle reasons of one GPU while the timed regions run.  Reads NVML in this process (a thread
+    that samples every 10 ms; the first sample is taken synchronously in start(), so that even a timed region of a
+    few milliseconds has its record); where NVML cannot be loaded it falls back to `nvidia-smi -lms 50`, whose output
+    is block-buffered and can therefore miss short runs -- `source` and `why` say which path ran and why a record is
+    empty."""
     FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
     NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    # NVML clocks-event (throttle) reason bits
+    BITS = {"sw_power_cap": 0x4, "hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40}
 
-    def __init__(self, index):
+    def __init__(self, index, pci_bus_id=None):
         self.index = index
+        self.pci_bus_id = pci_bus_id
         self.proc = None
         self.out = None
+        self.nvml = None
+        self.handle = None
+        self.thread = None
+        self.stop_flag = False
+        self.sm, self.mx, self.reasons = [], [], set()
+        self.why = None
+
+    def _sample(self):
+        n = self.nvml
+        self.sm.append(float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM)))
+        self.mx.append(float(n.nvmlDeviceGetMaxClockInfo(self.handle, n.NVML_CLOCK_SM)))
+        get = getattr(n, "nvmlDeviceGetCurrentClocksEventReasons", None) or n.nvmlDeviceGetCurrentClocksThrottleReasons
+        mask = int(get(self.handle))
+        for name, bit in self.BITS.items():
+            if mask & bit:
+                self.reasons.add(name)
+
+    def _loop(self):
+        while not self.stop_flag:
+            try:
+                self._sample()
+            except Exception as exc:  # keep what was sampled so far
+                self.why = "NVML sampling stopped: %r" % (exc,)
+                return
+            time.sleep(0.01)
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            try:
+                self.handle = pynvml.nvmlDeviceGetHandleByPciBusId(self.pci_bus_id.encode() if self.pci_bus_id else b"")
+            except Exception:
+                self.handle = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self._sample()
+            import threading
+            self.thread = threading.Thread(target=self._loop, daemon=True)
+            self.thread.start()
+            return
+        except Exception as exc:
+            self.nvml = None
+            self.why = "NVML unavailable (%r); fell back to nvidia-smi -lms 50" % (exc,)
         self.out = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.FIELDS,
                  "--format=csv,noheader,nounits", "-lms", "50"], stdout=self.out, stderr=subprocess.DEVNULL)
-        except OSError:
+        except OSError as exc:
             self.proc = None
+            self.why += "; nvidia-smi could not be started (%r)" % (exc,)
 
     def stop(self):
-        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
-        if self.proc is None:
-            return res
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except subprocess.TimeoutExpired:
-            self.proc.kill()
-        self.out.flush()
-        self.out.seek(0)
-        sm, mx, reasons = [], [], set()
-        for ln in self.out:
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) < 7:
-                continue
+        res = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0, "source": None, "why": None}
+        if self.nvml is not None:
             try:
-                sm.append(float(f[0]))
-                mx.append(float(f[1]))
-            except ValueError:
-                continue
-            for name, val in zip(self.NAMES, f[3:7]):
-                if val == "Active":
-                    reasons.add(name)
-        self.out.close()
-        os.unlink(self.out.name)
+                self._sample()                               # one more under the last timed region's tail
+            except Exception:
+                pass
+            self.stop_flag = True
+            if self.thread is not None:
+                self.thread.join(timeout=2)
+            res["source"] = "nvml (in-process, 10 ms)"
+            sm, mx, reasons = self.sm, self.mx, self.reasons
+        else:
+            res["source"] = "nvidia-smi -lms 50"
+            sm, mx, reasons = [], [], set()
+            if self.proc is not None:
+                self.proc.terminate()
+                try:
+                    self.proc.wait(timeout=5)
+                except subprocess.TimeoutExpired:
+                    self.proc.kill()
+                self.out.flush()
+                self.out.seek(0)
+                for ln in self.out:
+                    f = [x.strip() for x in ln.split(",")]
+                    if len(f) < 7:
+                        continue
+                    try:
+                        sm.append(float(f[0]))
+                        mx.append(float(f[1]))
+                    except ValueError:
+                        continue
+                    for name, val in zip(self.NAMES, f[3:7]):
+                        if val == "Active":
+                            reasons.add(name)
+                self.out.close()
+                os.unlink(self.out.name)
         if sm:
             res.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), reasons=sorted(reasons),
                        samples=len(sm))
+        res["why"] = self.why if sm else (self.why or "no sample arrived before the timed regions ended")
         return res
 
 
@@ -167,14 +229,17 @@ def _host_threads_for(w, cores):
 
 def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
     """The oracle's hybrid tier (T1, Eq.24; oracle.hybrid_layers with numpy's FFT, fp64), AS IT STANDS,
-    on the host cores, one state.  The binary128 tensor rows are prebuilt (setup, like hfft_build_tensor on the GPU);
-    everything else hybrid_layers does is inside the timing: the forward FFT of M (once per call), and per target
-    layer the 2-D FFT of the 6 nz padded tensor planes, the z-sum and the inverse FFT.  numpy's FFT and einsum run on
-    ONE thread (`cores_timed`); the all-cores figure runs the same calls, one target-layer chunk per thread.
+    on the host cores, one state -- like for like with the GPU arm ("tensor bank pre-built, setup
+    excluded"): the binary128 tensor rows AND their in-plane spectra (oracle.tensor_spectrum, what hfft_build_tensor
+    does on the GPU) are built before the timing and handed over through `nhat=`; inside the timing are the forward
+    FFT of M (once per call) and, per target layer, the z-sum of Eq.24 and the inverse FFT.  The figure that also pays
+    the tensor planes' 2-D FFT on every evaluation (hybrid_layers called with `rows=` only, as rounds 1-2 timed it)
+    is reported beside it as `with_tensor_fft`.  numpy's FFT and einsum run on ONE thread (`cores_timed`); the
+    all-cores figure runs the same calls, one target-layer chunk per thread.
 
-    C1-C3: whole evaluations (every target layer).  C4 / C5: a bounded sample -- calls with target layers [0] and
-    [0, 1] give the per-layer and the once-per-evaluation time; evaluation = once + nz * per_layer (the tensor row of
-    layer 0 stands in for both sampled layers: the timing does not depend on the values)."""
+    C1-C3: whole evaluations (every target layer).  C4 / C5: a bounded sample, EXTRAPOLATED -- calls with target layers
+    [0] and [0, 1] give the per-layer and the once-per-evaluation time; evaluation = once + nz * per_layer (the tensor
+    row of layer 0 stands in for both sampled layers: the timing does not depend on the values)."""
     import oracle as O
     from concurrent.futures import ThreadPoolExecutor
     m = w.m_rounded([0])[0]
@@ -187,10 +252,18 @@ def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
         row0 = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, 0)
         rows = {i: row0 for i in range(w.nz)}
     setup = time.perf_counter() - t0
+    t0 = time.perf_counter()
+    if full:
+        nhat = {i: O.tensor_spectrum(rows[i], w.nx, w.ny, "fft") for i in range(w.nz)}
+    else:
+        nhat0 = O.tensor_spectrum(row0, w.nx, w.ny, "fft")
+        nhat = {i: nhat0 for i in range(w.nz)}
+    setup_fft = time.perf_counter() - t0
 
-    def call(layers):
+    def call(layers, prebuilt=True):
+        kw = {"nhat": nhat} if prebuilt else {"rows": rows}
         t = time.perf_counter()
-        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, list(layers), dft="fft", rows=rows)
+        O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m, w.Ms, list(layers), dft="fft", **kw)
         return time.perf_counter() - t
 
     def repeat(fn, n_fixed):
@@ -211,6 +284,7 @@ def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
     if full:
         ts = repeat(lambda: call(range(w.nz)), steps)
         t_eval = float(np.mean(ts))
+        t_eval_fft = float(np.mean([call(range(w.nz), False) for _ in range(max(1, min(3, len(ts))))]))
         chunks = [list(range(w.nz))[t::nthr] for t in range(nthr)]
 
         def par():
@@ -222,14 +296,18 @@ def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
         t_eval_all = float(np.mean(tp))
         sample = ("whole evaluations (all %d target layers) of one state: mean of %d runs of %.4f s"
                   % (w.nz, len(ts), t_eval))
-        runs, s_per_step = len(ts), t_eval
+        formula = None
+        runs, s_timed = len(ts), float(np.sum(ts))
     else:
         n = steps if steps is not None else 3
-        t1 = float(np.median(repeat(lambda: call([0]), n)))
-        t2 = float(np.median(repeat(lambda: call([0, 1]), n)))
+        a1, a2 = repeat(lambda: call([0]), n), repeat(lambda: call([0, 1]), n)
+        t1, t2 = float(np.median(a1)), float(np.median(a2))
         per = max(t2 - t1, 1e-9)
         once = max(t1 - per, 0.0)
         t_eval = once + w.nz * per
+        f1, f2 = call([0], False), call([0, 1], False)
+        per_f = max(f2 - f1, 1e-9)
+        t_eval_fft = max(f1 - per_f, 0.0) + w.nz * per_f
 
         def par():
             t = time.perf_counter()
@@ -239,23 +317,59 @@ def oracle_timing(w, budget_s=20.0, steps=None, warmup=0):
         t_par = par()
         # nthr layers (each with its own forward FFT of M, as the call stands) in t_par seconds
         t_eval_all = t_par * w.nz / nthr
-        sample = ("target layers [0] (%.3f s) and [0, 1] (%.3f s) of %d, one state, median of %d calls each: "
-                  "evaluation = once-per-call %.3f s + nz * per-layer %.3f s" % (t1, t2, w.nz, n, once, per))
-        runs, s_per_step = 2 * n, t1 + t2
+        sample = ("target layers [0] (%.3f s) and [0, 1] (%.3f s) of %d, one state, median of %d calls each"
+                  % (t1, t2, w.nz, n))
+        formula = ("s_per_eval = once + nz * per_layer, per_layer = t[0,1] - t[0] = %.4f s, once = t[0] - per_layer = %.4f s, "
+                   "nz = %d: the %.1f s evaluation was not run" % (per, once, w.nz, t_eval))
+        runs, s_timed = 2 * n, float(np.sum(a1) + np.sum(a2))
     return {"value": 1.0 / t_eval, "unit": UNIT, "cores": 1, "cores_timed": 1, "cores_available": cores,
-            "kind": "oracle", "s_per_eval": t_eval,
-            "sample": sample + "; oracle.hybrid_layers (numpy FFT, fp64) as it stands: tensor rows prebuilt (binary128, "
-                      "%.1f s on %d OpenMP threads, untimed), the tensor planes' 2-D FFT, the forward FFT of M, the "
-                      "z-sum and the inverse FFT inside the timing" % (setup, O.threads()),
+            "kind": "oracle", "s_per_eval": t_eval, "extrapolated": not full, "extrapolation": formula,
+            "timed_work": "bank_prebuilt: forward FFT of M, z-sum of Eq.24, inverse FFT (tensor rows and their spectra built "
+                          "beforehand, as hfft_build_tensor does for the GPU arm)",
+            "with_tensor_fft": {"value": 1.0 / t_eval_fft, "unit": UNIT, "s_per_eval": t_eval_fft, "extrapolated": not full,
+                                "what": "hybrid_layers given the tensor rows only: it also transforms the 6 nz padded "
+                                        "tensor planes of every target layer on every evaluation (the figure rounds 1-2 "
+                                        "printed as `value`)"},
+            "sample": sample + "; oracle.hybrid_layers (numpy FFT, fp64) as it stands; untimed setup: tensor rows (binary128, "
+                      "%.1f s on %d OpenMP threads) and their in-plane spectra (oracle.tensor_spectrum, %.1f s)"
+                      % (setup, O.threads(), setup_fft),
             "all_cores": {"value": 1.0 / t_eval_all, "unit": UNIT, "cores": nthr, "s_per_eval": t_eval_all,
+                          "extrapolated": not full,
                           "how": "the same calls, one chunk of target layers per thread (numpy releases the GIL)"},
-            "oracle_tensor_rows_s": setup, "_runs": runs, "_s_per_step": s_per_step}
+            "oracle_tensor_rows_s": setup, "oracle_tensor_spectra_s": setup_fft, "_runs": runs, "_s_timed": s_timed}
 
 
 def cpu_baseline(w, budget_s=20.0):
     r = oracle_timing(w, budget_s)
-    r.pop("_runs"); r.pop("_s_per_step")
+    r.pop("_runs"); r.pop("_s_timed")
     return r
+
+
+def traffic_entry(workload_name, storage, root=None):
+    """(DRAM bytes per launch of the coupling kernel, where the figure comes from) out of profiles/traffic.json, or
+    (None, why).  An entry counts only while the source files that define its kernel still hash to what they did at
+    the capture: a changed kernel prints traffic = null (with the reason) instead of a stale number."""
+    import hashlib
+    root = root or ROOT
+    tp = os.path.join(root, "profiles", "traffic.json")
+    if not os.path.exists(tp):
+        return None, "no profiles/traffic.json"
+    with open(tp) as fh:
+        ent = json.load(fh).get(workload_name, {}).get(storage)
+    if not isinstance(ent, dict):
+        return None, "no ncu --set full capture of this workload with the %s storage" % storage
+    files = ent.get("source_files") or []
+    hsh = hashlib.sha256()
+    try:
+        for f in files:
+            with open(os.path.join(root, f), "rb") as fh:
+                hsh.update(fh.read())
+    except OSError as exc:
+        return None, "stale: %s (%r)" % (ent.get("source"), exc)
+    if not files or hsh.hexdigest()[:16] != ent.get("source_sha16"):
+        return None, ("stale: %s changed since the capture of %s at commit %s (%s); capture again"
+                      % (", ".join(files) or "kernel sources", ent.get("kernel"), ent.get("git"), ent.get("source")))
+    return ent.get("coupling_dram_bytes_per_launch"), "%s; kernel %s, commit %s" % (ent.get("source"), ent.get("kernel"), ent.get("git"))
 
 
 def l2_mode(w):
@@ -263,8 +377,17 @@ def l2_mode(w):
     print the same `config`.  Workloads whose smallest storage (reciprocity + ky-mirror bank) exceeds twice the L2
     stream it every step; the small ones get a 256 MiB memset before every timed step."""
     small = algorithmic_bytes(w, None, True, True)["whole"] < (256 << 20)
-    return ("L2 flushed (256 MiB memset) before every timed step" if small
-            else "inputs larger than L2 (126 MB): the tensor bank and the spectra are streamed from HBM every step")
+    if small:
+        return "L2 flushed (256 MiB memset) before every timed step"
+    # the bank is larger than L2 in every such workload; the spectra M^ / H^ (one complex plane set) may or may not be
+    elem = 4 if w.precision == "f32" else 8
+    spectra = 3 * w.nz * w.B * 2 * w.ny * (w.nx + 1) * 2 * elem
+    if spectra < (126 << 20):
+        return ("inputs larger than L2 (126 MB): the tensor bank is streamed from HBM every step; the spectra (%d MB) fit L2 "
+                "and are served from it between the stages, so the coupling's achieved GB/s on algorithmic bytes is L2-assisted"
+                % (spectra // 1000000))
+    return ("inputs larger than L2 (126 MB): the tensor bank and the spectra (%d MB) are streamed from HBM every step"
+            % (spectra // 1000000))
 
 
 def run_reference(args, w):
@@ -281,19 +404,63 @@ def run_reference(args, w):
     elif w.nx * w.ny * w.nz > 64 * 64 * 6:
         steps, warmup = max(1, min(args.steps, 5)), min(args.warmup, 1)
     r = oracle_timing(w, steps=steps, warmup=warmup)
-    runs, s_per_step = r.pop("_runs"), r.pop("_s_per_step")
+    runs, s_timed = r.pop("_runs"), r.pop("_s_timed")
     value = r["value"]
+    # One line, one meaning per key: `steps` / `warmup` are what RAN (the request is echoed beside them), `value` and
+    # `ms_per_step` describe one whole evaluation (value = 1000 / ms_per_step); where that evaluation is extrapolated
+    # from a bounded sample (C4, C5) the line says so and `timed_s` is the wall time of the calls actually timed.
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step, "higher_is_better": True,
+        "steps": steps if full else runs, "warmup": warmup, "ms_per_step": 1e3 * r["s_per_eval"], "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(w),
         "cpu_baseline": r,
-        "steps_run": steps, "warmup_run": warmup, "oracle_calls_timed": runs,
+        "extrapolated": r["extrapolated"], "extrapolation": r["extrapolation"],
+        "step_is": "one whole evaluation" if full else "one sampled oracle call (target layers [0] or [0, 1]); ms_per_step is "
+                   "the extrapolated whole evaluation, not the duration of such a call",
+        "steps_requested": args.steps, "warmup_requested": args.warmup, "oracle_calls_timed": runs, "timed_s": s_timed,
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
+
+
+def measure_pcie(torch, m_host, m, h, h_host, nbytes):
+    """What the PCIe link gives for the end-to-end step's own transfers, without any kernel: the pinned host -> device
+    copy of m and the device -> pinned host copy of h, the sizes and buffers of the e2e region, issued back to back on
+    two streams so that both directions run at once (as they do in the hfft_demag_host_async pipeline).  Returns GB/s
+    per direction with both directions busy, and each direction alone."""
+    cur = torch.cuda.current_stream()
+    s_in, s_out = torch.cuda.Stream(), torch.cuda.Stream()
+    iters = int(max(5, min(200, (1 << 30) // max(nbytes, 1))))
+
+    def run(do_in, do_out):
+        torch.cuda.synchronize()
+        e0 = torch.cuda.Event(enable_timing=True)
+        e1 = torch.cuda.Event(enable_timing=True)
+        e0.record(cur)
+        ends = []
+        for on, st, fn in ((do_in, s_in, lambda: m.copy_(m_host, non_blocking=True)),
+                           (do_out, s_out, lambda: h_host.copy_(h, non_blocking=True))):
+            if not on:
+                continue
+            st.wait_event(e0)
+            with torch.cuda.stream(st):
+                for _ in range(iters):
+                    fn()
+                ev = torch.cuda.Event()
+                ev.record(st)
+                ends.append(ev)
+        for ev in ends:
+            cur.wait_event(ev)
+        e1.record(cur)
+        torch.cuda.synchronize()
+        return iters * nbytes / (e0.elapsed_time(e1) * 1e-3) / 1e9
+
+    run(True, True)                                      # warm-up
+    return {"both_directions_gbs_per_direction": run(True, True), "h2d_alone_gbs": run(True, False),
+            "d2h_alone_gbs": run(False, True), "bytes_per_copy": nbytes, "copies_per_direction": iters,
+            "how": "pinned cudaMemcpyAsync of the step's own buffers on two streams, no kernels, CUDA events"}
 
 
 def max_over_ranks(times_ms, device="cpu"):
@@ -467,11 +634,20 @@ def main():
             flush.zero_()
         plan.demag(m, Ms, h)
 
-    for _ in range(warmup):
+    # clocks are sampled from the warm-up on (under load), through every timed region
+    props = torch.cuda.get_device_properties(local_rank)
+    try:
+        bus = "%08x:%02x:%02x.0" % (props.pci_domain_id, props.pci_bus_id, props.pci_device_id)
+    except AttributeError:
+        bus = None
+    sampler = ClockSampler(local_rank, bus)
+    if warmup > 0:                                       # the first sample is taken with the GPU already at work
         step()
-    sampler = ClockSampler(local_rank)
-    barrier()
+        torch.cuda.synchronize()
     sampler.start()
+    for _ in range(max(0, warmup - 1)):
+        step()
+    barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     # ---- timed region 1: device-resident inputs ----
     if flush is None:
@@ -564,6 +740,7 @@ def main():
     ms_e2e = ev0.elapsed_time(ev1)
     barrier()
     clocks = sampler.stop()
+    pcie = measure_pcie(torch, m_host, m, h, h_host, nbytes)     # after the timed regions; h_host keeps the same field
 
     assert bool(torch.isfinite(h).all()) and bool(torch.isfinite(h_host).all())
     ms_total, ms_e2e, ms_e2e_serial = max_over_ranks([ms_total, ms_e2e, ms_e2e_serial], device="cuda")
@@ -575,29 +752,28 @@ def main():
         coup_ms = float(stage_ms[hb.STAGE_NAMES.index("coupling")])
         achieved = ab["coupling"] / (coup_ms * 1e-3) / 1e9 if coup_ms > 0 else None
         # DRAM bytes per launch of the coupling kernel from the committed ncu --set full capture of this workload and
-        # storage (not re-measured here: ncu cannot run inside a timed bench)
-        traffic, traffic_src = None, None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
-        if os.path.exists(tp):
-            with open(tp) as fh:
-                tj = json.load(fh).get(w.name, {})
-            storage = ("zfft" if dedup == 4 else "class" if dedup else "batched" if w.B > 1 else
-                       "symv" if symv else "recip" if recip else "mirror" if mirror else "plain")
-            ent = tj.get(storage) if isinstance(tj.get(storage), dict) else None
-            if ent:
-                traffic, traffic_src = ent.get("coupling_dram_bytes_per_launch"), ent.get("source")
+        # storage (not re-measured here: ncu cannot run inside a timed bench); null once the kernel's sources changed
+        storage = ("zfft" if dedup == 4 else "class" if dedup else "batched" if w.B > 1 else
+                   "symv" if symv else "recip" if recip else "mirror" if mirror else "plain")
+        traffic, traffic_src = traffic_entry(w.name, storage)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": steps, "warmup": warmup,
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": w.precision, "data": "synthetic",
             "config": workload_config(w),
             "clocks": {"sm_mhz": clocks["sm_mhz"], "sm_max_mhz": clocks["sm_max_mhz"], "reasons": clocks["reasons"],
-                       "samples": clocks["samples"]},
+                       "samples": clocks["samples"], "source": clocks["source"], "why": clocks["why"]},
             "e2e": {"value": whole_job_value(world, w.B, e2e_steps, ms_e2e), "unit": UNIT,
                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps,
                     "api": "hfft_demag_host_async + hfft_host_join (per step: pinned host m -> device, 5 kernels, "
                            "device h -> pinned host; copies of neighbouring steps overlap the kernels)",
-                    "serialised_hfft_demag_host": whole_job_value(world, w.B, e2e_steps, ms_e2e_serial)},
+                    "serialised_hfft_demag_host": whole_job_value(world, w.B, e2e_steps, ms_e2e_serial),
+                    # "PCIe-bound" as a number: bytes per second and direction of the e2e region over what the link
+                    # gives for the same copies with no kernels in between (rank 0's link)
+                    "gbs_per_direction": nbytes * e2e_steps / (ms_e2e * 1e-3) / 1e9,
+                    "pcie_gbs_measured": pcie["both_directions_gbs_per_direction"],
+                    "frac_of_pcie": nbytes * e2e_steps / (ms_e2e * 1e-3) / 1e9 / pcie["both_directions_gbs_per_direction"],
+                    "pcie": pcie},
             "gpu_launches": plan.info.launches_per_demag * steps,
             "roofline": {"bound": "hbm", "kernel": "coupling_symv_kernel (S3, reciprocity + ky-mirror bank read once)" if symv
                          else "coupling_kernel (S3)", "achieved": achieved, "peak": peak,
@@ -605,7 +781,13 @@ def main():
                          "frac_of_nominal_8TBs": achieved / 8000.0 if achieved else None,
                          "algorithmic_bytes_per_launch": ab["coupling"], "avg_launch_ms": coup_ms,
                          "stored_bank_bytes": int(plan.info.bank_bytes),
-                         "traffic": traffic, "traffic_source": traffic_src},
+                         "traffic": traffic, "traffic_source": traffic_src,
+                         # the same launch time against the DRAM bytes ncu counted (cold L2) instead of the bytes the
+                         # method needs: where they differ, L2 serves part of the stream in a running evaluation
+                         "achieved_dram": traffic / (coup_ms * 1e-3) / 1e9 if traffic and coup_ms > 0 else None,
+                         "frac_dram": traffic / (coup_ms * 1e-3) / 1e9 / peak if traffic and coup_ms > 0 else None,
+                         "achieved_is": "algorithmic bytes / launch time" + ("" if ab["whole"] >= (2 << 30) else
+                                        " (L2-assisted: bank + spectra are within a few L2 sizes, part of M^ / H^ never leaves L2)")},
             "stages_ms": {n: float(v) for n, v in zip(hb.STAGE_NAMES, stage_ms)},
             "whole_eval": {"algorithmic_bytes": ab["whole"], "roofline_ms_at_peak": ab["whole"] / peak / 1e6,
                            "ms_per_step": ms_step, "ratio_to_roofline": ms_step / (ab["whole"] / peak / 1e6)},

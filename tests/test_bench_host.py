@@ -53,3 +53,10 @@ def test_reference_arm_prints_the_contract_line_on_config_1():
     assert cb["kind"] == "oracle" and cb["cores_timed"] == 1 and cb["value"] == line["value"] and "all_cores" in cb
     assert line["e2e"] == {"value": line["value"], "unit": bench.UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert line["gpu_launches"] == 0
+    # one meaning per key: the steps that ran, a whole evaluation per step, value = 1000 / ms_per_step, nothing extrapolated
+    assert line["steps"] == 3 and line["steps_requested"] == 3 and line["extrapolated"] is False and line["extrapolation"] is None
+    assert abs(line["value"] * line["ms_per_step"] / 1e3 - 1.0) < 1e-9
+    assert abs(line["timed_s"] - line["steps"] * line["ms_per_step"] / 1e3) < 1e-9
+    # like for like: `value` times the evaluation with the tensor spectra pre-built; the evaluation that also
+    # transforms the tensor planes is reported beside it and is the slower one
+    assert cb["with_tensor_fft"]["s_per_eval"] > cb["s_per_eval"] and "oracle_tensor_spectra_s" in cb
