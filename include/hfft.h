@@ -36,6 +36,11 @@
  *
  * Array layout (all calls): [B][3][nz][ny][nx], x fastest, component order
  * (x,y,z), element type float (HFFT_F32) or double (HFFT_F64), 16-byte aligned.
+ *
+ * Environment variables read by the library (A/B measurements only; none is needed for normal use, each is read
+ * once per process): HFFT_NO_PDL=1 launches the kernels of an evaluation in plain stream order instead of with
+ * programmatic dependent launch; HFFT_ZFFT_FORM=reg|smem forces the register or the shared-memory form of the
+ * z-FFT coupling kernel (hfft_plan_set_dedup mode 3) instead of the choice by layer count.  Results do not change.
  */
 #ifndef HFFT_H
 #define HFFT_H
@@ -170,7 +175,10 @@ hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
  *          (info.mirror == 2: saves memory, not time -- the second use of an entry is a
  *          second read).
  *   on = 0: never.
- * hfft_update_dz rebuilds the whole bank in these modes.  Must be called before
+ * hfft_update_dz rebuilds the WHOLE bank in these modes (every stored S_pq carries dz_p; C4: 0.22 s per update
+ * instead of a partial rebuild) -- and on = 2 is the default, so a thickness sweep on a large fp32 stack of 8 to 64
+ * layers should call hfft_plan_set_recip(plan, 0) first: the ky-mirror bank it then uses is twice as large and
+ * hfft_update_dz rewrites only the pairs that change.  Must be called before
  * hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
@@ -179,8 +187,9 @@ hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);
  * PAPER.md:177-178): stages S2, S3 and S4 run as ONE kernel in which a CTA takes the kx column of all 3 nz planes --
  * forward y transforms, coupling in shared memory, inverse y transforms -- so that M^ / H^ never reach global memory
  * and hfft_demag enqueues 3 kernels instead of 5 (info.fused == 1, info.launches_per_demag == 3).  It needs the plain
- * bank (no ky-mirror, reciprocity or deduplicated storage), the column 3 nz x 2ny complex plus the transform rows
- * within 222 KB of shared memory, nz <= 32, and no batched coupling.
+ * bank (no ky-mirror, reciprocity or deduplicated storage), two columns of 3 nz x 2ny complex plus the transform rows
+ * within 222 KB of shared memory (the only bound on nz: e.g. nz <= 126 at ny = 16 and nz <= 15 at ny = 128 in fp32),
+ * and no batched coupling.
  *   mode = 1 (default): automatic -- on the small grids (those too small for the wide-tile / mirror storage), which
  *          are bound by kernel launches; large grids keep the staged path with its smaller banks, which is faster
  *          there (measured: profiles/r02_fusion.md).
@@ -289,7 +298,9 @@ hfft_status hfft_host_join(hfft_plan *plan, void *stream);
  * `stream` and synchronises it before returning (frees its scratch memory).
  * Errors: EINVAL (k out of range, dz_new not positive / finite), ESTATE (tensor
  * not built), EUNSUPPORTED (deduplicated bank: use hfft_plan_set_dedup(plan, 0)),
- * ENOMEM, ECUDA (the plan then needs hfft_build_tensor again).
+ * ENOMEM, ECUDA (the plan then needs hfft_build_tensor again); ESTATE also while evaluations of
+ * hfft_demag_host_async are outstanding (they read the bank on the plan's own streams): call hfft_host_join
+ * first.  The same holds for a second hfft_build_tensor on a built plan.
  */
 hfft_status hfft_update_dz(hfft_plan *plan, int k, double dz_new, void *stream);
 

@@ -13,6 +13,8 @@ using namespace hfft;
 namespace {
 thread_local std::string g_create_error;
 constexpr int kMaxProfileCalls = 256;
+const char* kPipeBusy =
+    ": evaluations of hfft_demag_host_async are outstanding (they use the plan's spectra and bank); call hfft_host_join first";
 }  // namespace
 
 struct hfft_plan {
@@ -443,6 +445,9 @@ hfft_status hfft_plan_set_buffers(hfft_plan* plan, void* bank, void* workspace) 
 
 hfft_status hfft_build_tensor(hfft_plan* plan, void* stream) {
     if (!plan) return HFFT_EINVAL;
+    // a rebuild rewrites the bank (and clears the spectra) on the caller's stream while the pipeline's own compute
+    // stream may still be reading them
+    if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_build_tensor") + kPipeBusy);
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
     if ((e = cudaSetDevice(plan->device)) != cudaSuccess) return fail_cuda(plan, "cudaSetDevice", e);
@@ -583,9 +588,6 @@ static hfft_status demag_checked(hfft_plan* plan, const void* m, const double* M
     return plan->prec == HFFT_F32 ? demag_impl<float>(plan, m, Ms, h, st) : demag_impl<double>(plan, m, Ms, h, st);
 }
 
-static const char* kPipeBusy =
-    ": evaluations of hfft_demag_host_async are outstanding (they share the plan's spectra); call hfft_host_join first";
-
 hfft_status hfft_demag(hfft_plan* plan, const void* m, const double* Ms, void* h, void* stream) {
     if (!plan) return HFFT_EINVAL;
     if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_demag") + kPipeBusy);
@@ -604,6 +606,7 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
     if (k < 0 || k >= plan->nz) return fail(plan, HFFT_EINVAL, "hfft_update_dz: layer index out of range");
     if (!(dz_new > 0) || !isfinite(dz_new)) return fail(plan, HFFT_EINVAL, "hfft_update_dz: dz must be positive and finite");
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_update_dz: call hfft_build_tensor first");
+    if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_update_dz") + kPipeBusy);
     if (plan->dedup)
         return fail(plan, HFFT_EUNSUPPORTED, "hfft_update_dz: the bank is deduplicated; create the plan with hfft_plan_set_dedup(plan, 0)");
     cudaStream_t st = (cudaStream_t)stream;
@@ -645,6 +648,7 @@ hfft_status hfft_update_dz_static(hfft_plan* plan, int k, double dz_new, void* s
     if (k < 0 || k >= plan->nz) return fail(plan, HFFT_EINVAL, "hfft_update_dz_static: layer index out of range");
     if (!(dz_new > 0) || !isfinite(dz_new)) return fail(plan, HFFT_EINVAL, "hfft_update_dz_static: dz must be positive and finite");
     if (!plan->built) return fail(plan, HFFT_ESTATE, "hfft_update_dz_static: call hfft_build_tensor first");
+    if (plan->pipe_unjoined) return fail(plan, HFFT_ESTATE, std::string("hfft_update_dz_static") + kPipeBusy);
     if (plan->dedup)
         return fail(plan, HFFT_EUNSUPPORTED, "hfft_update_dz_static: the bank is deduplicated; create the plan with hfft_plan_set_dedup(plan, 0)");
     if (plan->recip && !plan->d_invdz) return fail(plan, HFFT_ESTATE, "hfft_update_dz_static: 1/dz table missing; rebuild the plan");

@@ -37,15 +37,21 @@ template <typename V> class PerDevice {
   public:
     bool get(int dev, long long key, V& out) {
         std::lock_guard<std::mutex> lock(mu_);
-        auto it = map_.find(std::make_pair(dev, key));
-        if (it == map_.end()) return false;
-        out = it->second;
-        return true;
+        return get_locked(dev, key, out);
     }
     void set(int dev, long long key, const V& v) {
         std::lock_guard<std::mutex> lock(mu_);
         map_[std::make_pair(dev, key)] = v;
     }
+    // for read-modify-write sequences that must not interleave between host threads (ctas_per_sm_cached)
+    std::mutex& mutex() { return mu_; }
+    bool get_locked(int dev, long long key, V& out) const {
+        auto it = map_.find(std::make_pair(dev, key));
+        if (it == map_.end()) return false;
+        out = it->second;
+        return true;
+    }
+    void set_locked(int dev, long long key, const V& v) { map_[std::make_pair(dev, key)] = v; }
   private:
     std::mutex mu_;
     std::map<std::pair<int, long long>, V> map_;
@@ -54,25 +60,28 @@ template <typename V> class PerDevice {
 // CTAs per SM of `kernel` launched with (threads, smem) on the current device, opting in to smem > 48 KB first.
 // The opt-in is one attribute per (kernel, device) that every call overwrites: it is only ever raised (key -1 of the
 // cache holds the value in force), so that a launch whose occupancy is cached never finds it lowered by a later,
-// smaller configuration.
+// smaller configuration.  The look-up of the value in force, cudaFuncSetAttribute and the update of key -1 happen
+// under ONE lock: two host threads that bring the same kernel up with different shared-memory sizes cannot leave the
+// attribute at the smaller value while the cache records the larger one.
 template <typename K>
 inline cudaError_t ctas_per_sm_cached(K kernel, int threads, size_t smem, PerDevice<int>& cache, int& occ) {
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     const long long key = ((long long)threads << 32) | (long long)smem;
-    if (cache.get(dev, key, occ)) return cudaSuccess;
+    std::lock_guard<std::mutex> lock(cache.mutex());
+    if (cache.get_locked(dev, key, occ)) return cudaSuccess;
     int opted = 48 * 1024;
-    cache.get(dev, -1, opted);
+    cache.get_locked(dev, -1, opted);
     if ((int)smem > opted) {
         if ((e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)) != cudaSuccess)
             return e;
-        cache.set(dev, -1, (int)smem);
+        cache.set_locked(dev, -1, (int)smem);
     }
     int nb = 0;
     if ((e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, kernel, threads, smem)) != cudaSuccess) return e;
     occ = nb < 1 ? 1 : nb;
-    cache.set(dev, key, occ);
+    cache.set_locked(dev, key, occ);
     return cudaSuccess;
 }
 

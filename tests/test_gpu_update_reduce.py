@@ -180,6 +180,11 @@ def test_pipelined_host_path_matches_plain_host_path(hb):
     torch.cuda.synchronize()
     for m in ms:                                     # five calls back to back, nothing synchronised in between
         got.append(plan.demag_host_async(m, w.Ms))
+    # until the join, nothing may rewrite the bank or the spectra the pipeline's own streams are still using
+    for call in (lambda: plan.update_dz(1, 2.0), lambda: plan.update_dz_static(1, 2.0), plan.build_tensor):
+        with pytest.raises(hb.HfftError) as e:
+            call()
+        assert e.value.status == hb.ESTATE and "hfft_host_join" in str(e.value)
     plan.host_join()
     torch.cuda.synchronize()
     for a, b in zip(got, want):
