@@ -223,28 +223,30 @@ def _full_layer_check(hb, w, layers, states=(0,), ncells=40, tol=None, expect=No
         info = hb.plan_info(plan.handle)
         for key, val in expect.items():
             assert getattr(info, key) == val, (key, getattr(info, key), val)
-    states = list(states)
-    m_sel = w.m_rounded(states)                                           # [len(states)][3][nz][ny][nx], fp64
+    # states: one list for every layer, or {layer: states} (C5: all layers of one state, one layer of several states)
+    states_of = (lambda i: list(states[i])) if isinstance(states, dict) else (lambda i: list(states))
     rng = np.random.default_rng(w.seed)
     err_t1, err_t0, scale = 0.0, 0.0, 0.0
     diffs = []
     for i in layers:
+        sel = states_of(i)
+        m_sel = w.m_rounded(sel)                                          # [len(sel)][3][nz][ny][nx], fp64
         Nrow = O.tensor_row(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, i)
         ref = O.hybrid_layers(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m_sel, w.Ms, [i], dft="fft", rows={i: Nrow})
         ref = ref[:, 0]                                                   # [states][3][ny][nx]
         scale = max(scale, float(np.abs(ref).max()))
-        got = np.stack([h[b, :, i].double().cpu().numpy() for b in states])
+        got = np.stack([h[b, :, i].double().cpu().numpy() for b in sel])
         diffs.append(float(np.abs(got - ref).max()))
         # corners, edges and random interior cells against the definition (direct sum)
         cells = np.concatenate([[0, w.nx - 1, (w.ny - 1) * w.nx, w.ny * w.nx - 1, (w.ny // 2) * w.nx + w.nx // 2],
                                 rng.choice(w.nx * w.ny, size=ncells - 5, replace=False)]).astype(np.int32)
-        for t, b in enumerate(states):
+        for t, b in enumerate(sel):
             H0 = O.direct_cells(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, m_sel[t], w.Ms, i, cells, Nrow=Nrow)
             g = got[t].reshape(3, -1)[:, cells].T
             err_t0 = max(err_t0, float(np.abs(g - H0).max()))
             # the oracle's two tiers agree far below the tolerance being tested
             assert np.abs(ref[t].reshape(3, -1)[:, cells].T - H0).max() <= 1e-11 * scale
-        del Nrow, ref
+        del Nrow, ref, m_sel
     plan.close()
     err_t1 = max(diffs) / scale
     err_t0 /= scale
@@ -276,16 +278,20 @@ def _uniform_average_check(hb, w, tol, **plan_kw):
 
 
 def test_config3_256x256x16_fp32_full_layers(hb):
-    """C3: three whole target layers (bottom, interior, top), every cell."""
+    """C3: six whole target layers spread over the stack (bottom and top included), every cell, through the kernel
+    bench.py times (reciprocity bank read once by coupling_symv_kernel: info.mirror == 3, no deduplication)."""
     w = W.config(3)
-    _full_layer_check(hb, w, layers=[0, 9, w.nz - 1])
+    _full_layer_check(hb, w, layers=[0, 3, 6, 9, 12, w.nz - 1], expect={"mirror": 3, "dedup": 0})
     _uniform_average_check(hb, w, 2e-6)
 
 
 def test_config4_256x256x64_fp32_full_layers(hb):
-    """C4, the headline configuration: an interior layer and the top layer nz - 1, every cell."""
+    """C4, the headline configuration: eight whole target layers, every cell -- one from eight different strips of
+    four layers of the symmetric-matvec layout (bottom, top and six in between), so that the tile walk, the ring
+    wrap-around over about a thousand tiles per CTA and the two-buffer prefetch are checked on rows that different
+    warps produce.  Asserts that the plan is the one bench.py times (info.mirror == 3, no deduplication)."""
     w = W.config(4)
-    _full_layer_check(hb, w, layers=[37, w.nz - 1], ncells=32)
+    _full_layer_check(hb, w, layers=[0, 5, 14, 23, 28, 37, 46, w.nz - 1], ncells=32, expect={"mirror": 3, "dedup": 0})
     _uniform_average_check(hb, w, 2e-6)
 
 
@@ -299,6 +305,9 @@ def test_config4_equal_thickness_variant_full_layers_zfft(hb):
 
 
 def test_config5_512x512x8_batch32_fp32_full_layer(hb):
-    """C5 (B = 32 states per call): one whole target layer for the first and the last state."""
+    """C5 (B = 32 states per call, the batched coupling kernel): all eight target layers of state 0, and layer 3 for
+    four states spread over the batch (first, two interior, last) -- every cell."""
     w = W.config(5)
-    _full_layer_check(hb, w, layers=[3], ncells=24, states=(0, 31))
+    states = {i: (0,) for i in range(w.nz)}
+    states[3] = (0, 10, 21, 31)
+    _full_layer_check(hb, w, layers=list(range(w.nz)), ncells=24, states=states, expect={"mirror": 0, "dedup": 0, "fused": 0, "tile_k": 32})  # tile_k 32 + B > 1: coupling_batched_kernel
