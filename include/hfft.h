@@ -175,10 +175,8 @@ hfft_status hfft_plan_set_mirror(hfft_plan *plan, int on);
  *          (info.mirror == 2: saves memory, not time -- the second use of an entry is a
  *          second read).
  *   on = 0: never.
- * hfft_update_dz rebuilds the WHOLE bank in these modes (every stored S_pq carries dz_p; C4: 0.22 s per update
- * instead of a partial rebuild) -- and on = 2 is the default, so a thickness sweep on a large fp32 stack of 8 to 64
- * layers should call hfft_plan_set_recip(plan, 0) first: the ky-mirror bank it then uses is twice as large and
- * hfft_update_dz rewrites only the pairs that change.  Must be called before
+ * hfft_update_dz rewrites, in these modes too, only the stored blocks whose layer pair has the changed layer
+ * between or at its two layers (the other blocks and the layout's zero padding are left alone).  Must be called before
  * hfft_build_tensor / hfft_plan_set_buffers.  Errors: EINVAL, ESTATE.
  */
 hfft_status hfft_plan_set_recip(hfft_plan *plan, int on);

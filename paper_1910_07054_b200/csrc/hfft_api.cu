@@ -623,9 +623,10 @@ hfft_status hfft_update_dz(hfft_plan* plan, int k, double dz_new, void* stream) 
         return fail(plan, HFFT_ENOMEM, std::string("cudaMalloc(setup scratch): ") + cudaGetErrorString(e));
     }
     std::string msg;
-    // reciprocity storage: every stored S_pq = dz_p R_pq of a changed pair is rebuilt from its representative (the
-    // class tables select them), which here means the whole bank; and the 1 / dz table changes
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, plan->recip ? -1 : k, st, msg);
+    // reciprocity storage: the stored orientation S_pq = dz_p R_pq of every changed pair is rebuilt (row_runs picks
+    // them out of the pair table; the untouched blocks of the symv layout keep their values, no memset); and the
+    // 1 / dz table changes
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, k, st, msg);
     if (e == cudaSuccess && plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) msg = "1/dz table";
     cudaError_t e2 = cudaStreamSynchronize(st);
     cudaFree(scratch);
@@ -676,7 +677,7 @@ hfft_status hfft_update_dz_static(hfft_plan* plan, int k, double dz_new, void* s
     // The array still holds the previous call's intermediates.  build_bank writes every table it reads (interface
     // coordinates, class table, lattice and stencil values, transforms) and clears, on `st`, the real-space planes
     // whose padding must be zero -- the same as with the uninitialised memory cudaMalloc hands out.
-    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, plan->recip ? -1 : k, st, msg);
+    e = build_bank(g, plan->bank, scratch, plan->tw_x64, plan->twt_x64, plan->twt_y64, k, st, msg);
     if (e == cudaSuccess && plan->recip && (e = upload_inv_dz(plan)) != cudaSuccess) msg = "1/dz table";   // d_invdz exists: a copy only
     cudaError_t e2 = cudaStreamSynchronize(st);
     if (e != cudaSuccess || e2 != cudaSuccess) {

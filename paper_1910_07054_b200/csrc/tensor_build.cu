@@ -215,7 +215,9 @@ size_t build_scratch_bytes(const BuildGeom& g) { return scratch_layout(g).total;
 // Source layers j of target row i whose tensor has to be evaluated, as inclusive runs [j0, j1].
 //  - hfft_update_dz (changed >= 0): N_ij depends on (dz_i, dz_j, zeta_i - zeta_j) only, so pairs
 //    on one side of the changed layer keep their tensor;
-//  - deduplicated bank (g.pair_class): only the representative pair of every tensor class.
+//  - deduplicated bank (g.pair_class): only the representative pair of every tensor class;
+//  - reciprocity storage (g.pair_class = slot of the unordered pair): the stored orientation of every pair, and with
+//    changed >= 0 only the pairs that straddle or contain the changed layer.
 static std::vector<std::pair<int, int>> row_runs(const BuildGeom& g, int changed, int i) {
     const int nz = g.nz;
     std::vector<std::pair<int, int>> runs;
@@ -227,6 +229,10 @@ static std::vector<std::pair<int, int>> row_runs(const BuildGeom& g, int changed
     }
     for (int j = 0; j < nz; ++j) {
         if (g.class_rep[g.pair_class[i * nz + j]] != i * nz + j) continue;
+        // reciprocity storage + hfft_update_dz: of the stored orientations only those whose pair has the changed layer
+        // between (or at) its two layers get a new tensor; S_pq = dz_p R_pq changes with dz_p only for p == changed,
+        // which is one of them
+        if (changed >= 0 && !((i <= changed && changed <= j) || (j <= changed && changed <= i))) continue;
         if (!runs.empty() && runs.back().second == j - 1) runs.back().second = j;
         else runs.push_back({j, j});
     }
