@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--recip", type=int, default=None, help="hfft_plan_set_recip (default: the library's)")
     ap.add_argument("--dedup", type=int, default=None, help="hfft_plan_set_dedup mode (default: the library's, 1)")
     ap.add_argument("--fusion", type=int, default=None, help="hfft_plan_set_fusion mode (default: the library's, 1)")
+    ap.add_argument("--update-dz", action="store_true",
+                    help="time one thickness update (hfft_update_dz / hfft_update_dz_static) against the full tensor build")
     ap.add_argument("--all-configs", action="store_true",
                     help="run every config (1, 2, 2f64, 3, 4, 4eq, 5) in a process of its own and write the bench lines, "
                          "with their clocks, as a markdown table + JSON lines to --out")
@@ -527,6 +529,52 @@ def sweep_nz():
 SEED_SWEEP = 191007054
 
 
+def update_dz_timing():
+    """SURVEY 8f-1 / PAPER.md:205-211 (the tensor is rebuilt at every Newton step of the thickness optimisation): wall
+    time of one thickness update -- hfft_update_dz (scratch from cudaMalloc / cudaFree per call) and, where the plan fits
+    the fixed 32 MiB scratch, hfft_update_dz_static (no allocation) -- against the full hfft_build_tensor, per bank
+    storage.  Both update calls synchronise their stream, so host wall time is the time of the call.  Median of 5."""
+    import torch
+    from paper_1910_07054_b200 import binding as hb
+    saf = W.small(64, 64, 5, precision="f64", seed=1, dz=np.array([5.0, 1.0, 5.0, 1.0, 3.0]))
+    cases = [("SAF disc grid 64x64x5 f64 (PAPER.md:205-211)", saf, 2, dict()),
+             ("C2 64x64x6 f32", W.config(2), 3, dict()),
+             ("C3 256x256x16 f32, reciprocity bank (default)", W.config(3), 8, dict()),
+             ("C3 256x256x16 f32, ky-mirror bank (recip 0)", W.config(3), 8, dict(recip=0)),
+             ("C4 256x256x64 f32, reciprocity bank (default), middle layer", W.config(4), 32, dict()),
+             ("C4 256x256x64 f32, reciprocity bank (default), bottom layer", W.config(4), 0, dict()),
+             ("C4 256x256x64 f32, ky-mirror bank (recip 0), middle layer", W.config(4), 32, dict(recip=0))]
+    for name, w, k, kw in cases:
+        plan = hb.Plan(w.nx, w.ny, w.nz, w.dx, w.dy, w.dz, w.precision, dedup=0, **kw)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        plan.build_tensor()
+        torch.cuda.synchronize()
+        build_s = time.perf_counter() - t0
+        info = hb.plan_info(plan.handle)
+
+        def med(fn):
+            ts = []
+            for r in range(6):
+                dz_new = w.dz[k] * (1.1 if r % 2 == 0 else 1.0)
+                torch.cuda.synchronize()
+                t = time.perf_counter()
+                fn(k, dz_new)
+                ts.append(time.perf_counter() - t)
+            return float(np.median(ts[1:]))
+        upd = med(plan.update_dz)
+        fits = info.setup_scratch_bytes <= hb.STATIC_SCRATCH_BYTES
+        sta = med(plan.update_dz_static) if fits else None
+        changed = sum(1 for i in range(w.nz) for j in range(i, w.nz) if i <= k <= j)
+        print(json.dumps({"case": name, "layer": k, "mirror": info.mirror, "bank_GB": info.bank_bytes / 1e9,
+                          "setup_scratch_MB": info.setup_scratch_bytes / 1e6, "build_tensor_s": build_s,
+                          "update_dz_s": upd, "update_dz_static_s": sta,
+                          "unordered_pairs_changed": changed, "unordered_pairs": w.nz * (w.nz + 1) // 2}), flush=True)
+        plan.close()
+        del plan
+        torch.cuda.empty_cache()
+
+
 def workload_config(w):
     l2 = l2_mode(w)
     return {"workload": w.name, "nx": w.nx, "ny": w.ny, "nz": w.nz, "batch": w.B, "precision": w.precision,
@@ -554,7 +602,7 @@ def all_configs(args):
     with open(args.out, "w") as fh:
         fh.write("# bench.py --all-configs --steps %d --warmup %d\n\n" % (args.steps, args.warmup))
         fh.write("Command: `python bench.py --all-configs --steps %d --warmup %d --out %s` (one B200; every config in a "
-                 "process of its own; clocks sampled with nvidia-smi during the timed regions).\n\n" % (args.steps, args.warmup, args.out))
+                 "process of its own; clocks sampled through NVML from the warm-up on, bench.ClockSampler).\n\n" % (args.steps, args.warmup, args.out))
         fh.write("| config | ms / call | evals/s | e2e evals/s | S1 / S2 / S3 / S4 / S5 ms | S3 roofline (bound, achieved / peak = frac) "
                  "| whole / roofline | bank | SM MHz (median / max) | throttle reasons |\n|---|---:|---:|---:|---|---|---:|---|---|---|\n")
         for d in lines:
@@ -573,6 +621,9 @@ def main():
     args = parse_args()
     if args.sweep_nz:
         sweep_nz()
+        return
+    if args.update_dz:
+        update_dz_timing()
         return
     if args.all_configs:
         all_configs(args)
